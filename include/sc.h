@@ -1,0 +1,144 @@
+/*
+ * sc.h -- C ABI of libsc: real-space convolution of a HEALPix RING map with a compact,
+ * radially symmetric kernel on one NVIDIA B200 (sm_100a).
+ *
+ * The operation (BASELINE.json north_star; the "real-space portion" that the paper runs on the
+ * GPU -- PAPER.md:66 section 2, Fig. 1 caption -- i.e. "convolving a ... map with a
+ * radial kernel", with the real-space kernel truncated at theta_cut):
+ *
+ *     out_b(p) = Omega_pix * SUM_{q : theta_pq <= theta_max} K(cos theta_pq) * m_b(q),
+ *     Omega_pix = 4 pi / N_pix,  N_pix = 12 nside^2,  b = 0 .. B-1 (maps sharing one kernel).
+ *
+ * Inclusion (reading R4) is decided exactly as the fp64 test
+ *     z_p z_q + (s_p s_q) cos(phi_p - phi_q) >= cos(theta_max)
+ * evaluated in IEEE double without FMA contraction (the self pair is included); K is the linear
+ * interpolant of the caller's table in cos(theta) (PAPER.md:106 speaks of interpolating the
+ * real-space kernel from nodes; node placement here is uniform in cos theta, reading R5);
+ * products and sums are fp32 on the device ("single-precision arithmetic in the GPU",
+ * PAPER.md:124).
+ *
+ * Conventions
+ *   - Nothing throws or aborts across this boundary: every entry point returns an sc_status and
+ *     leaves its outputs untouched on failure.
+ *   - "HOST" / "DEVICE" below say where a pointer must live.  The library never allocates or
+ *     frees memory the caller passes in; a plan owns its own device tables.
+ *   - A plan belongs to the CUDA device that was current when it was created and is immutable
+ *     afterwards; it may be used from one stream at a time.
+ *   - There is no CPU fallback: without a usable CUDA device sc_plan_create returns SC_ERR_CUDA.
+ */
+#ifndef SC_H
+#define SC_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sc_plan sc_plan; /* opaque */
+
+typedef enum {
+    SC_OK = 0,
+    SC_ERR_INVALID_ARG = 1, /* NULL where not allowed, nside < 1, n_table < 2, theta_max out of range, B < 1 ... */
+    SC_ERR_UNSUPPORTED = 2, /* NESTED ordering; 12 nside^2 >= 2^31; knife-edge list overflow */
+    SC_ERR_ALLOC = 3,       /* host or device allocation failed */
+    SC_ERR_CUDA = 4         /* no device / a CUDA call failed (sc_last_cuda_error() names it) */
+} sc_status;
+
+enum { SC_ORDER_RING = 0, SC_ORDER_NESTED = 1 };
+
+/* Which kernels sc_convolve may use (debug / measurement knob; results are the same operation). */
+enum {
+    SC_PATH_AUTO = 0,     /* fastest available for every ring (default) */
+    SC_PATH_GENERIC = 1   /* one thread per output pixel everywhere (the simple reference kernel) */
+};
+
+/*
+ * sc_plan_create -- precompute everything that depends only on (nside, kernel, theta_max).
+ *   plan       HOST  out: receives the new plan (unchanged on failure).
+ *   nside      HEALPix resolution, >= 1, need not be a power of two; 12 nside^2 < 2^31.
+ *   ordering   SC_ORDER_RING.  SC_ORDER_NESTED returns SC_ERR_UNSUPPORTED.
+ *   ktable     HOST  n_table doubles, K sampled at x_i = c + i (1 - c)/(n_table - 1),
+ *              c = cos(theta_max), i.e. ktable[0] = K(cos theta_max), ktable[n_table-1] = K(1).
+ *              Copied; the caller may free it after the call.
+ *   n_table    >= 2.
+ *   theta_max  radians, 0 < theta_max <= pi/2.
+ *   max_batch  >= 1: largest B later passed to sc_convolve (larger B still works, in chunks).
+ * Work done: ring geometry tables (fp64 and fp32), the device interpolation table, per-ring
+ * input-ring intervals, and one audit pass on the GPU that counts all pairs and collects
+ * "knife-edge" pairs (|dot - c| below a few ulp) whose inclusion is then decided on the host
+ * with the host libm (DESIGN.md section "Bit-exact inclusion").  Synchronous.
+ */
+sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *ktable,
+                         int n_table, double theta_max, int max_batch);
+
+/*
+ * sc_convolve -- the hot path.  Enqueues the convolution of B maps on `cuda_stream` and returns
+ * without synchronising the host.
+ *   in_maps    HOST array of B DEVICE pointers, each to N_pix fp32 values (RING order),
+ *              16-byte aligned.
+ *   out_maps   HOST array of B DEVICE pointers, each to N_pix fp32 values, 16-byte aligned;
+ *              must not alias any input.  Fully overwritten.
+ *   B          >= 1.
+ *   cuda_stream  a cudaStream_t (CUstream) passed as void*; NULL = the legacy default stream.
+ * Map values are plain numbers: no bad-pixel sentinel is interpreted (paper silent).
+ */
+sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *const *out_maps,
+                      int B, void *cuda_stream);
+
+/*
+ * sc_convolve_host -- the same operation with HOST buffers (the end-to-end call): copies the B
+ * input maps to plan-owned device staging buffers, runs sc_convolve, copies the results back and
+ * synchronises.  in/out: HOST arrays of B HOST pointers to N_pix fp32 each (pinned memory makes
+ * the copies faster but is not required).
+ */
+sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host,
+                           float *const *out_maps_host, int B);
+
+/* Destroy a plan and free its device memory.  NULL is allowed. */
+sc_status sc_plan_destroy(sc_plan *plan);
+
+/* Select the kernel path used by later sc_convolve calls on this plan (SC_PATH_*). */
+sc_status sc_plan_set_path(sc_plan *plan, int path);
+
+/*
+ * sc_plan_info -- facts about a plan.  Any output pointer may be NULL.
+ *   npix            12 nside^2
+ *   total_pairs     number of included (p, q) pairs over the whole sphere, self pairs included
+ *                   (from the audit pass)
+ *   cos_theta_max   the threshold c used by the inclusion test
+ *   n_knife_edge    number of pairs that were decided on the host
+ */
+sc_status sc_plan_info(const sc_plan *plan, int64_t *npix, int64_t *total_pairs,
+                       double *cos_theta_max, int64_t *n_knife_edge);
+
+/*
+ * sc_debug_neighbour_counts -- verification only, not part of the timed path.  For every pixel
+ * p writes the number of included neighbours to count_dev[p] and, if sig_dev != NULL, the sum of
+ * the neighbours' RING indices to sig_dev[p].  Both DEVICE pointers, N_pix entries.
+ * Uses the same inclusion code as sc_convolve.  Asynchronous on cuda_stream.
+ */
+sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uint64_t *sig_dev,
+                                    void *cuda_stream);
+
+/*
+ * sc_debug_stats -- numbers gathered by the audit pass at plan creation (HOST outputs, may be NULL):
+ *   n_uncertain   pairs whose fp32 table coordinate fell inside the guard band and were therefore
+ *                 re-decided in fp64 on the device
+ *   max_t_err     max |t_fp32 - t_fp64| (table cells) seen over those pairs
+ *   guard_band    half-width of the guard band (table cells)
+ */
+sc_status sc_debug_stats(const sc_plan *plan, int64_t *n_uncertain, double *max_t_err,
+                         double *guard_band);
+
+/* Kernel launches enqueued by the last sc_convolve / sc_convolve_host on this plan. */
+int sc_last_launch_count(const sc_plan *plan);
+
+const char *sc_status_string(sc_status s);
+/* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
+const char *sc_last_cuda_error(void);
+/* Library version, e.g. "sc 0.1 (sm_100a)". */
+const char *sc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SC_H */

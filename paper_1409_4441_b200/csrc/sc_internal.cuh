@@ -1,0 +1,116 @@
+// sc_internal.cuh -- structures and device helpers shared by the kernels of libsc (product code;
+// shares nothing with oracle/).  See include/sc.h for the operation and DESIGN.md for the design.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sc {
+
+constexpr int kMaxB = 4;          // maps per launch (larger batches are chunked by the host)
+constexpr int kTabPad = 64;       // zero entries appended to the device table (t clamps to tmax+1)
+
+// Device view of a plan.  Passed to kernels by value.
+struct Dev {
+    int nside, nrings, npix, ncap;        // ncap = 2 N (N-1): pixels in one polar cap (rings 1..N-1)
+    int ntab;                             // n: table nodes
+    float tmax;                           // n-1: table coordinate of theta_max
+    float eps;                            // guard half-width in table cells: |t - tmax| <= eps -> fp64 decision
+    float omega;                          // 4 pi / N_pix
+    double c;                             // cos(theta_max), host libm
+    double scale;                         // (n-1)/(1-c): t = (1 - dot) * scale
+    double ke_band;                       // |dot - c| <= ke_band -> knife-edge (host decides)
+    // ring tables, index = ring number - 1, rings 1 .. 4N-1
+    const double *z, *s, *phi0, *dphi;    // canonical fp64 geometry (R4)
+    const int *start, *npr;               // first pixel, pixels in ring
+    const int *rlo, *rhi;                 // candidate input-ring interval (1-based, inclusive)
+    // device interpolation table: K(t) = tab[i].x + t * tab[i].y for t in [i, i+1), t = (1-dot)*scale
+    const float2 *tab;
+    // knife-edge overrides decided on the host, sorted by key = p * npix + q
+    const unsigned long long *ke_key;
+    const unsigned char *ke_in;
+    int n_ke;
+};
+
+// Audit outputs (plan creation / debug only)
+struct Audit {
+    unsigned long long *total_pairs;      // sum of counts
+    unsigned long long *n_uncertain;      // pairs decided in fp64
+    unsigned int *max_t_err_bits;         // max |t32 - t64| as float bits
+    unsigned long long *ke_list;          // recorded knife-edge pairs: key | (gpu verdict << 63)
+    unsigned int *ke_count;
+    unsigned int ke_cap;
+};
+
+struct Maps {
+    const float *in[kMaxB];
+    float *out[kMaxB];
+};
+
+// ---------------------------------------------------------------------------------------------
+// device helpers
+// ---------------------------------------------------------------------------------------------
+
+// ring (1-based) and in-ring index of RING pixel p
+__device__ __forceinline__ int ring_of_pixel(const Dev &P, int p, int &k) {
+    const int N = P.nside;
+    int ring;
+    if (p < P.ncap) {
+        int i = (int)(0.5 * (1.0 + sqrt(1.0 + 2.0 * (double)p)));
+        while (i > 1 && 2 * i * (i - 1) > p) --i;
+        while (2 * i * (i + 1) <= p) ++i;
+        ring = i;
+    } else if (p < P.npix - P.ncap) {
+        ring = N + (p - P.ncap) / (4 * N);
+    } else {
+        const int pm = P.npix - 1 - p;
+        int i = (int)(0.5 * (1.0 + sqrt(1.0 + 2.0 * (double)pm)));
+        while (i > 1 && 2 * i * (i - 1) > pm) --i;
+        while (2 * i * (i + 1) <= pm) ++i;
+        ring = 4 * N - i;
+    }
+    k = p - P.start[ring - 1];
+    return ring;
+}
+
+// The canonical fp64 inclusion quantity, R4: every operation individually rounded
+// (no FMA contraction), phi = phi0 + k*dphi with k the in-ring index in [0, n).
+__device__ __forceinline__ double canonical_dot(const Dev &P, int rp, int kp, int rq, int kq) {
+    const double phip = __dadd_rn(P.phi0[rp - 1], __dmul_rn((double)kp, P.dphi[rp - 1]));
+    const double phiq = __dadd_rn(P.phi0[rq - 1], __dmul_rn((double)kq, P.dphi[rq - 1]));
+    const double cd = cos(__dsub_rn(phip, phiq));
+    return __dadd_rn(__dmul_rn(P.z[rp - 1], P.z[rq - 1]),
+                     __dmul_rn(__dmul_rn(P.s[rp - 1], P.s[rq - 1]), cd));
+}
+
+// Exact decision for one pair (slow path).  If `au` is given the pair is also audited.
+static __device__ __noinline__ bool exact_included(const Dev &P, int rp, int kp, int rq, int kq, float t32,
+                                            const Audit *au) {
+    const double dot = canonical_dot(P, rp, kp, rq, kq);
+    bool in = dot >= P.c;
+    const bool knife = fabs(dot - P.c) <= P.ke_band;
+    if (knife) {
+        const unsigned long long key =
+            (unsigned long long)(P.start[rp - 1] + kp) * (unsigned long long)P.npix +
+            (unsigned long long)(P.start[rq - 1] + kq);
+        int lo = 0, hi = P.n_ke - 1;
+        while (lo <= hi) {                 // host verdicts win
+            const int mid = (lo + hi) >> 1;
+            const unsigned long long km = P.ke_key[mid];
+            if (km == key) { in = P.ke_in[mid] != 0; break; }
+            if (km < key) lo = mid + 1; else hi = mid - 1;
+        }
+        if (au && au->ke_list) {
+            const unsigned int slot = atomicAdd(au->ke_count, 1u);
+            if (slot < au->ke_cap) au->ke_list[slot] = key | ((unsigned long long)(dot >= P.c) << 63);
+        }
+    }
+    if (au) {
+        atomicAdd(au->n_uncertain, 1ull);
+        const double t64 = (1.0 - dot) * P.scale;
+        const float err = fabsf((float)((double)t32 - t64));
+        atomicMax(au->max_t_err_bits, __float_as_uint(err));
+    }
+    return in;
+}
+
+}  // namespace sc

@@ -1,0 +1,395 @@
+// sc_plan.cu -- host side of libsc: the C ABI of include/sc.h, plan construction (HEALPix RING
+// ring tables, device interpolation table, input-ring intervals, knife-edge audit) and kernel
+// dispatch.  Product code: shares nothing with oracle/.
+#include "../../include/sc.h"
+#include "sc_internal.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace sc {
+cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1, cudaStream_t st);
+cudaError_t launch_generic_count(const Dev &P, int *count_dev, unsigned long long *sig_dev, const Audit *au, cudaStream_t st);
+struct FastPlan;
+FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std::vector<double> &s,
+                           int max_batch, int *polar_rings, cudaError_t *err);
+void fast_plan_destroy(FastPlan *fp);
+cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches);
+}  // namespace sc
+
+namespace {
+thread_local std::string g_cuda_err;
+
+bool cuda_ok(cudaError_t e, const char *what) {
+    if (e == cudaSuccess) return true;
+    g_cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return false;
+}
+#define SC_CUDA(call) do { if (!cuda_ok((call), #call)) return SC_ERR_CUDA; } while (0)
+
+// One ring of the HEALPix RING scheme (Gorski et al. 2005; the paper only cites it, PAPER.md:76,
+// :216).  Canonical fp64 evaluation of DESIGN.md R4: this order of operations fixes the last bit
+// of z, s, phi0, dphi and therefore of the inclusion test.
+struct RingGeom { int start, n, shifted; double z, s, phi0, dphi; };
+
+RingGeom healpix_ring(int N, int i) {
+    RingGeom g;
+    const int64_t npix = 12LL * N * N;
+    if (i < N) {                                   // north polar cap
+        g.n = 4 * i;
+        g.start = (int)(2LL * i * (i - 1));
+        g.z = 1.0 - (double)((int64_t)i * i) / (3.0 * N * N);
+        g.shifted = 0;
+    } else if (i <= 3 * N) {                       // equatorial belt
+        g.n = 4 * N;
+        g.start = (int)(2LL * N * (N - 1) + (int64_t)(i - N) * 4 * N);
+        g.z = (2.0 * N - i) * 2.0 / (3.0 * N);
+        g.shifted = (i - N) & 1;
+    } else {                                       // south polar cap
+        const int64_t m = 4LL * N - i;
+        g.n = (int)(4 * m);
+        g.start = (int)(npix - 2 * m * (m + 1));
+        g.z = -(1.0 - (double)(m * m) / (3.0 * N * N));
+        g.shifted = 0;
+    }
+    g.s = std::sqrt((1.0 - g.z) * (1.0 + g.z));
+    g.dphi = 2.0 * M_PI / g.n;
+    g.phi0 = g.shifted ? 0.0 : 0.5 * g.dphi;
+    return g;
+}
+
+template <class T> sc_status upload(const std::vector<T> &h, T **d) {
+    *d = nullptr;
+    const size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(T);
+    if (!cuda_ok(cudaMalloc((void **)d, bytes), "cudaMalloc")) return SC_ERR_ALLOC;
+    if (!h.empty()) SC_CUDA(cudaMemcpy(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return SC_OK;
+}
+}  // namespace
+
+struct sc_plan {
+    sc::Dev dev{};
+    int device = 0;
+    int max_batch = 1;
+    int path = SC_PATH_AUTO;
+    int64_t total_pairs = 0, n_knife = 0, n_uncertain = 0;
+    double max_t_err = 0.0;
+    std::vector<RingGeom> rings;
+    std::vector<void *> owned;                 // device allocations
+    // end-to-end staging
+    float *stage_in = nullptr, *stage_out = nullptr;
+    int stage_maps = 0;
+    cudaStream_t own_stream = nullptr;
+    mutable int last_launches = 0;
+    sc::FastPlan *fast = nullptr;
+    int polar_rings = 0;                       // rings 1..polar_rings and their southern mirrors use the generic kernel
+};
+
+namespace {
+
+template <class T> sc_status upload_owned(sc_plan *pl, const std::vector<T> &h, const T **d) {
+    T *p = nullptr;
+    sc_status st = upload(h, &p);
+    if (st != SC_OK) return st;
+    pl->owned.push_back(p);
+    *d = p;
+    return SC_OK;
+}
+
+void pix_to_ring(const sc_plan *pl, int64_t p, int &ring, int &k) {
+    // largest ring with start <= p
+    int lo = 0, hi = (int)pl->rings.size() - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (pl->rings[mid].start <= p) lo = mid; else hi = mid - 1;
+    }
+    ring = lo + 1;
+    k = (int)(p - pl->rings[lo].start);
+}
+
+// Host verdict for a knife-edge pair: the canonical test with the host libm (R4).
+bool host_included(const sc_plan *pl, int64_t p, int64_t q) {
+    int rp, kp, rq, kq;
+    pix_to_ring(pl, p, rp, kp);
+    pix_to_ring(pl, q, rq, kq);
+    const RingGeom &P = pl->rings[rp - 1], &Q = pl->rings[rq - 1];
+    const double phip = P.phi0 + (double)kp * P.dphi;
+    const double phiq = Q.phi0 + (double)kq * Q.dphi;
+    const double ss = P.s * Q.s;
+    const double cd = std::cos(phip - phiq);
+    const double zz = P.z * Q.z;
+    const double sc = ss * cd;
+    const double dot = zz + sc;
+    return dot >= pl->dev.c;
+}
+
+sc_status run_audit(sc_plan *pl) {
+    using namespace sc;
+    const unsigned int cap = 1u << 20;
+    unsigned long long *d_tot = nullptr, *d_unc = nullptr, *d_list = nullptr;
+    unsigned int *d_err = nullptr, *d_cnt = nullptr;
+    if (!cuda_ok(cudaMalloc((void **)&d_tot, 8), "cudaMalloc") || !cuda_ok(cudaMalloc((void **)&d_unc, 8), "cudaMalloc") ||
+        !cuda_ok(cudaMalloc((void **)&d_err, 4), "cudaMalloc") || !cuda_ok(cudaMalloc((void **)&d_cnt, 4), "cudaMalloc") ||
+        !cuda_ok(cudaMalloc((void **)&d_list, (size_t)cap * 8), "cudaMalloc"))
+        return SC_ERR_ALLOC;
+    sc_status st = SC_OK;
+    do {
+        if (!cuda_ok(cudaMemset(d_tot, 0, 8), "memset") || !cuda_ok(cudaMemset(d_unc, 0, 8), "memset") ||
+            !cuda_ok(cudaMemset(d_err, 0, 4), "memset") || !cuda_ok(cudaMemset(d_cnt, 0, 4), "memset")) { st = SC_ERR_CUDA; break; }
+        Audit au{d_tot, d_unc, d_err, d_list, d_cnt, cap};
+        if (!cuda_ok(launch_generic_count(pl->dev, nullptr, nullptr, &au, 0), "audit launch")) { st = SC_ERR_CUDA; break; }
+        if (!cuda_ok(cudaDeviceSynchronize(), "audit sync")) { st = SC_ERR_CUDA; break; }
+        unsigned long long tot = 0, unc = 0; unsigned int errb = 0, n = 0;
+        cudaMemcpy(&tot, d_tot, 8, cudaMemcpyDeviceToHost);
+        cudaMemcpy(&unc, d_unc, 8, cudaMemcpyDeviceToHost);
+        cudaMemcpy(&errb, d_err, 4, cudaMemcpyDeviceToHost);
+        if (!cuda_ok(cudaMemcpy(&n, d_cnt, 4, cudaMemcpyDeviceToHost), "memcpy")) { st = SC_ERR_CUDA; break; }
+        if (n > cap) { st = SC_ERR_UNSUPPORTED; break; }   // too many knife-edge pairs to list
+        float errf; std::memcpy(&errf, &errb, 4);
+        pl->n_uncertain = (int64_t)unc;
+        pl->max_t_err = errf;
+        std::vector<unsigned long long> list(n);
+        if (n && !cuda_ok(cudaMemcpy(list.data(), d_list, (size_t)n * 8, cudaMemcpyDeviceToHost), "memcpy")) { st = SC_ERR_CUDA; break; }
+        std::sort(list.begin(), list.end(), [](unsigned long long a, unsigned long long b) {
+            return (a & ~(1ull << 63)) < (b & ~(1ull << 63)); });
+        std::vector<unsigned long long> keys; std::vector<unsigned char> verdict;
+        long long delta = 0;
+        for (unsigned int i = 0; i < n; ++i) {
+            const unsigned long long key = list[i] & ~(1ull << 63);
+            if (!keys.empty() && keys.back() == key) continue;
+            const bool gpu_in = (list[i] >> 63) != 0;
+            const bool host_in = host_included(pl, (int64_t)(key / (unsigned long long)pl->dev.npix),
+                                               (int64_t)(key % (unsigned long long)pl->dev.npix));
+            keys.push_back(key); verdict.push_back(host_in ? 1 : 0);
+            delta += (int)host_in - (int)gpu_in;
+        }
+        pl->n_knife = (int64_t)keys.size();
+        pl->total_pairs = (int64_t)tot + delta;
+        if (!keys.empty()) {
+            if ((st = upload_owned(pl, keys, &pl->dev.ke_key)) != SC_OK) break;
+            if ((st = upload_owned(pl, verdict, &pl->dev.ke_in)) != SC_OK) break;
+            pl->dev.n_ke = (int)keys.size();
+        }
+    } while (0);
+    cudaFree(d_tot); cudaFree(d_unc); cudaFree(d_err); cudaFree(d_cnt); cudaFree(d_list);
+    return st;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *sc_status_string(sc_status s) {
+    switch (s) {
+        case SC_OK: return "SC_OK";
+        case SC_ERR_INVALID_ARG: return "SC_ERR_INVALID_ARG";
+        case SC_ERR_UNSUPPORTED: return "SC_ERR_UNSUPPORTED";
+        case SC_ERR_ALLOC: return "SC_ERR_ALLOC";
+        case SC_ERR_CUDA: return "SC_ERR_CUDA";
+    }
+    return "SC_ERR_?";
+}
+
+const char *sc_last_cuda_error(void) { return g_cuda_err.c_str(); }
+const char *sc_version(void) { return "sc 0.1 (sm_100a)"; }
+
+sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *ktable, int n_table,
+                         double theta_max, int max_batch) {
+    if (!plan || !ktable || nside < 1 || n_table < 2 || max_batch < 1) return SC_ERR_INVALID_ARG;
+    if (!(theta_max > 0.0) || !(theta_max <= M_PI / 2)) return SC_ERR_INVALID_ARG;
+    if (ordering == SC_ORDER_NESTED) return SC_ERR_UNSUPPORTED;
+    if (ordering != SC_ORDER_RING) return SC_ERR_INVALID_ARG;
+    if (12LL * nside * nside >= (1LL << 31)) return SC_ERR_UNSUPPORTED;
+    if (n_table > (1 << 24)) return SC_ERR_UNSUPPORTED;
+    for (int i = 0; i < n_table; ++i) if (!std::isfinite(ktable[i])) return SC_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (!cuda_ok(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev < 1) {
+        if (g_cuda_err.empty()) g_cuda_err = "no CUDA device";
+        return SC_ERR_CUDA;
+    }
+
+    sc_plan *pl = new (std::nothrow) sc_plan;
+    if (!pl) return SC_ERR_ALLOC;
+    sc_status st = SC_OK;
+    do {
+        if (!cuda_ok(cudaGetDevice(&pl->device), "cudaGetDevice")) { st = SC_ERR_CUDA; break; }
+        pl->max_batch = max_batch;
+        const int N = nside, nr = 4 * N - 1;
+        sc::Dev &D = pl->dev;
+        D.nside = N; D.nrings = nr; D.npix = 12 * N * N; D.ncap = 2 * N * (N - 1);
+        D.ntab = n_table;
+        D.tmax = (float)(n_table - 1);
+        D.eps = 0.0625f + 4e-6f * (float)(n_table - 1);
+        D.omega = (float)(4.0 * M_PI / (double)D.npix);
+        D.c = std::cos(theta_max);
+        const double one_minus_c = 2.0 * std::sin(0.5 * theta_max) * std::sin(0.5 * theta_max);
+        D.scale = (double)(n_table - 1) / one_minus_c;
+        D.ke_band = std::ldexp(1.0, -50);
+        if (const char *e = std::getenv("SC_KNIFE_EDGE_BAND")) { const double v = std::atof(e); if (v > 0) D.ke_band = v; }
+
+        // ring tables
+        pl->rings.resize(nr);
+        std::vector<double> z(nr), s(nr), phi0(nr), dphi(nr);
+        std::vector<int> start(nr), npr(nr), rlo(nr), rhi(nr);
+        for (int i = 1; i <= nr; ++i) {
+            const RingGeom g = healpix_ring(N, i);
+            pl->rings[i - 1] = g;
+            z[i - 1] = g.z; s[i - 1] = g.s; phi0[i - 1] = g.phi0; dphi[i - 1] = g.dphi;
+            start[i - 1] = g.start; npr[i - 1] = g.n;
+        }
+        // candidate input rings of an output ring: closest approach of two rings is at equal
+        // azimuth, cos(theta - theta') = z z' + s s'.  Slack + one extra ring: a strict superset
+        // (the kernels re-test every ring and every pixel).
+        const double slack = 1e-9 + 2.0 * (double)D.eps / D.scale;
+        for (int i = 1; i <= nr; ++i) {
+            int lo = i, hi = i;
+            while (lo > 1 && z[i - 1] * z[lo - 2] + s[i - 1] * s[lo - 2] >= D.c - slack) --lo;
+            while (hi < nr && z[i - 1] * z[hi] + s[i - 1] * s[hi] >= D.c - slack) ++hi;
+            if (lo > 1) --lo;
+            if (hi < nr) ++hi;
+            rlo[i - 1] = lo; rhi[i - 1] = hi;
+        }
+        // device table in the reversed coordinate t = (1 - x) (n-1)/(1-c): node j of the device
+        // table is caller node n-1-j.  Cell [j, j+1): K = a_j + t b_j with b_j = T'_{j+1} - T'_j,
+        // a_j = T'_j - j b_j  (fp64, rounded once).  Zero padding after the last cell.
+        std::vector<float2> tab((size_t)n_table - 1 + sc::kTabPad);
+        for (int j = 0; j < n_table - 1; ++j) {
+            const double t0 = ktable[n_table - 1 - j], t1 = ktable[n_table - 2 - j];
+            const double b = t1 - t0, a = t0 - (double)j * b;
+            tab[j] = make_float2((float)a, (float)b);
+        }
+        for (size_t j = (size_t)n_table - 1; j < tab.size(); ++j) tab[j] = make_float2(0.f, 0.f);
+
+        if ((st = upload_owned(pl, z, &D.z)) != SC_OK) break;
+        if ((st = upload_owned(pl, s, &D.s)) != SC_OK) break;
+        if ((st = upload_owned(pl, phi0, &D.phi0)) != SC_OK) break;
+        if ((st = upload_owned(pl, dphi, &D.dphi)) != SC_OK) break;
+        if ((st = upload_owned(pl, start, &D.start)) != SC_OK) break;
+        if ((st = upload_owned(pl, npr, &D.npr)) != SC_OK) break;
+        if ((st = upload_owned(pl, rlo, &D.rlo)) != SC_OK) break;
+        if ((st = upload_owned(pl, rhi, &D.rhi)) != SC_OK) break;
+        if ((st = upload_owned(pl, tab, &D.tab)) != SC_OK) break;
+        D.ke_key = nullptr; D.ke_in = nullptr; D.n_ke = 0;
+
+        if ((st = run_audit(pl)) != SC_OK) break;
+
+        cudaError_t ferr = cudaSuccess;
+        pl->fast = sc::fast_plan_create(D, z, s, max_batch, &pl->polar_rings, &ferr);
+        if (ferr != cudaSuccess) { cuda_ok(ferr, "fast_plan_create"); st = SC_ERR_CUDA; break; }
+    } while (0);
+    if (st != SC_OK) { sc_plan_destroy(pl); return st; }
+    *plan = pl;
+    return SC_OK;
+}
+
+sc_status sc_plan_destroy(sc_plan *plan) {
+    if (!plan) return SC_OK;
+    if (plan->fast) sc::fast_plan_destroy(plan->fast);
+    for (void *p : plan->owned) cudaFree(p);
+    if (plan->stage_in) cudaFree(plan->stage_in);
+    if (plan->stage_out) cudaFree(plan->stage_out);
+    if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
+    delete plan;
+    return SC_OK;
+}
+
+sc_status sc_plan_set_path(sc_plan *plan, int path) {
+    if (!plan || (path != SC_PATH_AUTO && path != SC_PATH_GENERIC)) return SC_ERR_INVALID_ARG;
+    plan->path = path;
+    return SC_OK;
+}
+
+sc_status sc_plan_info(const sc_plan *plan, int64_t *npix, int64_t *total_pairs, double *cos_theta_max,
+                       int64_t *n_knife_edge) {
+    if (!plan) return SC_ERR_INVALID_ARG;
+    if (npix) *npix = plan->dev.npix;
+    if (total_pairs) *total_pairs = plan->total_pairs;
+    if (cos_theta_max) *cos_theta_max = plan->dev.c;
+    if (n_knife_edge) *n_knife_edge = plan->n_knife;
+    return SC_OK;
+}
+
+sc_status sc_debug_stats(const sc_plan *plan, int64_t *n_uncertain, double *max_t_err, double *guard_band) {
+    if (!plan) return SC_ERR_INVALID_ARG;
+    if (n_uncertain) *n_uncertain = plan->n_uncertain;
+    if (max_t_err) *max_t_err = plan->max_t_err;
+    if (guard_band) *guard_band = plan->dev.eps;
+    return SC_OK;
+}
+
+int sc_last_launch_count(const sc_plan *plan) { return plan ? plan->last_launches : 0; }
+
+sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *const *out_maps, int B,
+                      void *cuda_stream) {
+    if (!plan || !in_maps || !out_maps || B < 1) return SC_ERR_INVALID_ARG;
+    for (int b = 0; b < B; ++b) {
+        if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
+        if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return SC_ERR_INVALID_ARG;
+        for (int a = 0; a < B; ++a) if ((const float *)out_maps[b] == in_maps[a]) return SC_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const sc::Dev &D = plan->dev;
+    int launches = 0;
+    for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
+        const int nb = std::min(sc::kMaxB, B - b0);
+        sc::Maps io{};
+        for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
+        if (plan->path == SC_PATH_GENERIC || !plan->fast) {
+            SC_CUDA(sc::launch_generic_conv(D, io, nb, 0, D.npix, 0, 0, st));
+            ++launches;
+        } else {
+            // rings next to the poles: generic kernel; everything else: fast kernels
+            const int pr = plan->polar_rings;
+            if (pr > 0) {
+                const int np = 2 * pr * (pr + 1);          // pixels in rings 1..pr
+                SC_CUDA(sc::launch_generic_conv(D, io, nb, 0, np, D.npix - np, D.npix, st));
+                ++launches;
+            }
+            int nl = 0;
+            SC_CUDA(sc::fast_convolve(plan->fast, D, io, nb, st, &nl));
+            launches += nl;
+        }
+    }
+    plan->last_launches = launches;
+    return SC_OK;
+}
+
+sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, float *const *out_maps_host, int B) {
+    if (!plan || !in_maps_host || !out_maps_host || B < 1) return SC_ERR_INVALID_ARG;
+    for (int b = 0; b < B; ++b) if (!in_maps_host[b] || !out_maps_host[b]) return SC_ERR_INVALID_ARG;
+    const size_t npix = (size_t)plan->dev.npix;
+    if (plan->stage_maps < B) {
+        if (plan->stage_in) cudaFree(plan->stage_in);
+        if (plan->stage_out) cudaFree(plan->stage_out);
+        plan->stage_in = plan->stage_out = nullptr; plan->stage_maps = 0;
+        const int nm = std::max(B, plan->max_batch);
+        if (!cuda_ok(cudaMalloc((void **)&plan->stage_in, npix * 4 * nm), "cudaMalloc")) return SC_ERR_ALLOC;
+        if (!cuda_ok(cudaMalloc((void **)&plan->stage_out, npix * 4 * nm), "cudaMalloc")) return SC_ERR_ALLOC;
+        plan->stage_maps = nm;
+    }
+    if (!plan->own_stream) SC_CUDA(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
+    std::vector<const float *> in(B); std::vector<float *> out(B);
+    for (int b = 0; b < B; ++b) {
+        in[b] = plan->stage_in + npix * b; out[b] = plan->stage_out + npix * b;
+        SC_CUDA(cudaMemcpyAsync(plan->stage_in + npix * b, in_maps_host[b], npix * 4, cudaMemcpyHostToDevice, plan->own_stream));
+    }
+    sc_status st = sc_convolve(plan, in.data(), out.data(), B, plan->own_stream);
+    if (st != SC_OK) return st;
+    for (int b = 0; b < B; ++b)
+        SC_CUDA(cudaMemcpyAsync(out_maps_host[b], out[b], npix * 4, cudaMemcpyDeviceToHost, plan->own_stream));
+    SC_CUDA(cudaStreamSynchronize(plan->own_stream));
+    return SC_OK;
+}
+
+sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uint64_t *sig_dev, void *cuda_stream) {
+    if (!plan || !count_dev) return SC_ERR_INVALID_ARG;
+    SC_CUDA(sc::launch_generic_count(plan->dev, count_dev, (unsigned long long *)sig_dev, nullptr, (cudaStream_t)cuda_stream));
+    return SC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,281 @@
+"""GPU parity: the CUDA path (through the C ABI of include/sc.h) against the fp64 oracle, element by
+element, on the seeded inputs of workloads/gen.py.
+
+Bars (BASELINE.json north_star): neighbour enumeration bit-exact (per-pixel counts and index-sum
+signatures identical); fp32 outputs within relative-rms <= 1e-6 and max-abs <= 1e-5 * max|out|.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+from workloads import gen
+
+pytestmark = pytest.mark.gpu
+
+REL_RMS_TOL = 1e-6          # BASELINE.json north_star
+MAX_ABS_TOL = 1e-5          # times max|out|
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _totals():
+    rows = {}
+    with open(os.path.join(GOLD, "pair_totals.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                a = line.split()
+                rows[(int(a[0]), int(a[1]))] = int(a[2])
+    return rows
+
+
+@pytest.fixture(scope="module")
+def sc():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1409_4441_b200 as sc
+    return sc
+
+
+def _gpu_convolve(sc, plan, maps):
+    import torch
+    dm = [torch.from_numpy(np.ascontiguousarray(m, np.float32)).cuda() for m in maps]
+    out = plan.convolve(dm)
+    torch.cuda.synchronize()
+    return [o.cpu().numpy() for o in out]
+
+
+def _check_values(got, want, what):
+    """got fp32, want fp64 on the same pixels."""
+    want = np.asarray(want, np.float64)
+    err = got.astype(np.float64) - want
+    relrms = np.sqrt(np.mean(err ** 2) / np.mean(want ** 2))
+    maxabs = np.max(np.abs(err)) / np.max(np.abs(want))
+    print(f"{what}: rel-rms {relrms:.3e}  max-abs/max|out| {maxabs:.3e}")
+    assert relrms <= REL_RMS_TOL, (what, relrms)
+    assert maxabs <= MAX_ABS_TOL, (what, maxabs)
+
+
+def _check_counts(sc, plan, cnt_ref, sig_ref, sel=None):
+    cnt, sig = plan.neighbour_counts()
+    cnt, sig = cnt.cpu().numpy(), sig.cpu().numpy().view(np.uint64)
+    if sel is not None:
+        cnt, sig = cnt[sel], sig[sel]
+    np.testing.assert_array_equal(cnt, cnt_ref)
+    np.testing.assert_array_equal(sig, sig_ref)
+
+
+PATHS = ["auto", "generic"]
+
+
+def _set_path(sc, plan, path):
+    plan.set_path(sc.SC_PATH_GENERIC if path == "generic" else sc.SC_PATH_AUTO)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config1_full(sc, path):
+    """Nside 64, theta_max 3.4 deg: every pixel, values + counts + signatures + exact pair total."""
+    cfg = gen.config(1)
+    T, maps = gen.table_for(cfg), gen.maps_for(cfg)
+    ref, cnt, sig = O.convolve(cfg.nside, T, cfg.theta_max, maps)
+    with sc.Plan(cfg.nside, T, cfg.theta_max, cfg.batch) as plan:
+        _set_path(sc, plan, path)
+        info = plan.info()
+        assert info["total_pairs"] == _totals()[(64, 204)] == int(cnt.sum())
+        _check_counts(sc, plan, cnt, sig)
+        out = _gpu_convolve(sc, plan, maps)
+        _check_values(out[0], ref[0], f"cfg1/{path}")
+        assert sc.sc_last_launch_count(plan.handle) >= 1
+        print("audit:", info)
+        assert info["max_t_err"] < info["guard_band"]
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config2_full_batch2(sc, path):
+    """Nside 256, theta_max 1.5 deg, B = 2 (noise map + band-limited map): every pixel."""
+    cfg = gen.config(2)
+    T, maps = gen.table_for(cfg), gen.maps_for(cfg)
+    ref, cnt, sig = O.convolve(cfg.nside, T, cfg.theta_max, maps)
+    with sc.Plan(cfg.nside, T, cfg.theta_max, cfg.batch) as plan:
+        _set_path(sc, plan, path)
+        assert plan.info()["total_pairs"] == _totals()[(256, 90)] == int(cnt.sum())
+        _check_counts(sc, plan, cnt, sig)
+        out = _gpu_convolve(sc, plan, maps)
+        for b in range(2):
+            _check_values(out[b], ref[b], f"cfg2/{path}/map{b}")
+
+
+def _sampled_config(sc, ci, key, n_val, n_cnt, path="auto"):
+    cfg = gen.config(ci)
+    T, maps = gen.table_for(cfg), gen.maps_for(cfg)
+    sel_v = gen.sample_pixels(cfg.nside, n_val, seed=100 + ci)
+    sel_c = gen.sample_pixels(cfg.nside, n_cnt, seed=200 + ci)
+    ref, cnt_v, sig_v = O.convolve(cfg.nside, T, cfg.theta_max, maps, sel=sel_v)
+    cnt_c, sig_c = O.count(cfg.nside, cfg.theta_max, sel=sel_c)
+    with sc.Plan(cfg.nside, T, cfg.theta_max, cfg.batch) as plan:
+        _set_path(sc, plan, path)
+        info = plan.info()
+        print("audit:", info)
+        assert info["total_pairs"] == _totals()[key]
+        assert info["max_t_err"] < info["guard_band"]
+        cnt, sig = plan.neighbour_counts()
+        cnt, sig = cnt.cpu().numpy(), sig.cpu().numpy().view(np.uint64)
+        assert int(cnt.astype(np.int64).sum()) == _totals()[key]
+        np.testing.assert_array_equal(cnt[sel_c], cnt_c)
+        np.testing.assert_array_equal(sig[sel_c], sig_c)
+        np.testing.assert_array_equal(cnt[sel_v], cnt_v)
+        np.testing.assert_array_equal(sig[sel_v], sig_v)
+        out = _gpu_convolve(sc, plan, maps)
+        for b in range(cfg.batch):
+            # normalise by the statistics of the sampled reference (white-noise map: stationary)
+            _check_values(out[b][sel_v], ref[b], f"cfg{ci}/{path}/map{b}")
+            assert np.all(np.isfinite(out[b]))
+        return out
+
+
+def test_config3_sampled(sc):
+    """Nside 1024, theta_max 30': exact pair total over the sphere; counts on 200k and values on 20k
+    sampled pixels (poles, cap/belt boundaries, equator + seeded random)."""
+    _sampled_config(sc, 3, (1024, 30), 20000, 200000)
+
+
+def test_config4_sampled(sc):
+    """Nside 2048, theta_max 20', split-like oscillating kernel (the metric's configuration)."""
+    _sampled_config(sc, 4, (2048, 20), 20000, 200000)
+
+
+def test_config5_sampled_batch3(sc):
+    """Nside 2048, theta_max 60', B = 3."""
+    _sampled_config(sc, 5, (2048, 60), 4000, 50000)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_paths_agree_config3_rings(sc, path):
+    """Whole rings at Nside 1024 (several tiles + ragged tails): pole rings, a mid-cap ring, the
+    cap/belt boundary, a belt ring, the equator and their southern mirrors."""
+    cfg = gen.config(3)
+    T, maps = gen.table_for(cfg), gen.maps_for(cfg)
+    t = O.ring_table(cfg.nside)
+    N = cfg.nside
+    rings = [1, 2, 3, 7, 33, 100, 517, N - 1, N, N + 1, N + 40, 2 * N - 1, 2 * N, 2 * N + 1, 3 * N - 1, 3 * N,
+             3 * N + 1, 4 * N - 100, 4 * N - 2, 4 * N - 1]
+    sel = np.concatenate([np.arange(t["start"][r - 1], t["start"][r - 1] + t["npr"][r - 1]) for r in rings])
+    ref, cnt, sig = O.convolve(cfg.nside, T, cfg.theta_max, maps, sel=sel)
+    with sc.Plan(cfg.nside, T, cfg.theta_max, 1) as plan:
+        _set_path(sc, plan, path)
+        out = _gpu_convolve(sc, plan, maps)
+        _check_values(out[0][sel], ref[0], f"cfg3 rings/{path}")
+        # per ring too, so that a broken short ring cannot hide in the average
+        off = 0
+        scale = np.sqrt(np.mean(ref[0] ** 2))
+        for r in rings:
+            n = int(t["npr"][r - 1])
+            e = out[0][sel[off:off + n]].astype(np.float64) - ref[0][off:off + n]
+            assert np.sqrt(np.mean(e ** 2)) / scale <= REL_RMS_TOL, r
+            off += n
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_exact_integer_sums(sc, path):
+    """K == 1 table and small-integer maps: every product and sum is exact in fp32, so the output
+    equals fl32(fl32(sum) * fl32(Omega)) bit for bit iff the neighbour SET used by the convolution
+    kernels themselves is the oracle's (counts alone could not see a swapped pixel)."""
+    for nside, theta in ((64, 3.4 * gen.DEG), (128, 1.0 * gen.DEG), (37, 5.0 * gen.DEG)):
+        npix = 12 * nside * nside
+        rng = np.random.default_rng(nside)
+        m = rng.integers(-8, 9, size=npix).astype(np.float32)
+        T = np.ones(64)
+        ref, cnt, _ = O.convolve(nside, T, theta, [m])
+        omega = np.float32(4 * np.pi / npix)
+        s = np.rint(ref[0] / (4 * np.pi / npix))
+        assert np.max(np.abs(s)) < 2 ** 24
+        want = s.astype(np.float32) * omega
+        with sc.Plan(nside, T, theta, 1) as plan:
+            _set_path(sc, plan, path)
+            out = _gpu_convolve(sc, plan, [m])
+        np.testing.assert_array_equal(out[0], want)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("nside,theta_deg,ntab", [(1, 60.0, 17), (2, 50.0, 2), (3, 89.9, 33), (5, 30.0, 100),
+                                                  (8, 75.0, 257), (16, 13.6, 1000), (32, 0.5, 64),
+                                                  (11, 7.0, 4096), (64, 90.0, 513)])
+def test_edge_geometries_full(sc, path, nside, theta_deg, ntab):
+    """Tiny and non-power-of-two Nside, pole-containing discs, whole-ring windows, discs up to a
+    hemisphere, 2-node tables, theta_max below the pixel spacing: all pixels, sets and values."""
+    npix = 12 * nside * nside
+    rng = np.random.default_rng(nside * 1000 + ntab)
+    T = rng.standard_normal(ntab)
+    maps = [rng.standard_normal(npix).astype(np.float32)]
+    theta = theta_deg * gen.DEG
+    ref, cnt, sig = O.convolve(nside, T, theta, maps)
+    with sc.Plan(nside, T, theta, 1) as plan:
+        _set_path(sc, plan, path)
+        assert plan.info()["total_pairs"] == int(cnt.sum())
+        _check_counts(sc, plan, cnt, sig)
+        out = _gpu_convolve(sc, plan, maps)
+    _check_values(out[0], ref[0], f"edge nside {nside} theta {theta_deg}/{path}")
+
+
+def test_identity_limit(sc):
+    """theta_max below the nearest-neighbour distance: count == 1, out = Omega * K(1) * m."""
+    nside, theta = 64, 0.2 * gen.DEG
+    npix = 12 * nside * nside
+    T = np.linspace(0.25, 3.0, 9)
+    m = gen.noise_map(npix, 42)
+    with sc.Plan(nside, T, theta, 1) as plan:
+        cnt, _ = plan.neighbour_counts()
+        assert int(cnt.min()) == 1 and int(cnt.max()) == 1
+        out = _gpu_convolve(sc, plan, [m])
+    want = (4 * np.pi / npix) * 3.0 * m.astype(np.float64)
+    np.testing.assert_allclose(out[0], want, rtol=3e-7, atol=0)
+
+
+def test_batch_chunking_and_host_entry(sc):
+    """B = 6 (> maps per launch) through sc_convolve, and the HOST-buffer entry sc_convolve_host,
+    give the same numbers as six single-map calls."""
+    cfg = gen.config(1)
+    T = gen.table_for(cfg)
+    maps = [gen.noise_map(cfg.npix, 50 + i) for i in range(6)]
+    with sc.Plan(cfg.nside, T, cfg.theta_max, 6) as plan:
+        single = [_gpu_convolve(sc, plan, [m])[0] for m in maps]
+        batch = _gpu_convolve(sc, plan, maps)
+        host = plan.convolve_host(maps)
+    ref, _, _ = O.convolve(cfg.nside, T, cfg.theta_max, maps)
+    for b in range(6):
+        np.testing.assert_array_equal(batch[b], single[b])
+        np.testing.assert_array_equal(host[b], single[b])
+        _check_values(batch[b], ref[b], f"batch6 map{b}")
+
+
+def test_knife_edge_host_adjudication(sc, monkeypatch):
+    """Widen the knife-edge band so that many pairs are decided on the host with the host libm;
+    sets must still equal the oracle's and the override list must be in use."""
+    monkeypatch.setenv("SC_KNIFE_EDGE_BAND", "1e-7")
+    nside, theta = 32, 6.0 * gen.DEG
+    npix = 12 * nside * nside
+    T = np.ones(16)
+    m = np.random.default_rng(3).integers(-8, 9, size=npix).astype(np.float32)
+    ref, cnt, sig = O.convolve(nside, T, theta, [m])
+    with sc.Plan(nside, T, theta, 1) as plan:
+        info = plan.info()
+        assert info["n_knife_edge"] > 0
+        assert info["total_pairs"] == int(cnt.sum())
+        _check_counts(sc, plan, cnt, sig)
+        out = _gpu_convolve(sc, plan, [m])
+    omega = np.float32(4 * np.pi / npix)
+    want = np.rint(ref[0] / (4 * np.pi / npix)).astype(np.float32) * omega
+    np.testing.assert_array_equal(out[0], want)
+
+
+def test_argument_errors_on_gpu(sc):
+    import torch
+    cfg = gen.config(1)
+    with sc.Plan(cfg.nside, gen.table_for(cfg), cfg.theta_max, 1) as plan:
+        a = torch.zeros(cfg.npix, device="cuda")
+        with pytest.raises(sc.ScError):            # aliasing
+            sc.sc_convolve(plan.handle, [a.data_ptr()], [a.data_ptr()])
+        with pytest.raises(sc.ScError):            # misaligned
+            sc.sc_convolve(plan.handle, [a.data_ptr() + 4], [torch.empty_like(a).data_ptr()])
+        with pytest.raises(sc.ScError):            # empty batch
+            sc.sc_convolve(plan.handle, [], [])
