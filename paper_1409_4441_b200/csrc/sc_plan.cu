@@ -20,6 +20,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
                            int max_batch, int *polar_rings, cudaError_t *err);
 void fast_plan_destroy(FastPlan *fp);
 cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches);
+bool fast_available(const FastPlan *fp, int B);
 }  // namespace sc
 
 namespace {
@@ -339,7 +340,7 @@ sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *c
         const int nb = std::min(sc::kMaxB, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
-        if (plan->path == SC_PATH_GENERIC || !plan->fast) {
+        if (plan->path == SC_PATH_GENERIC || !sc::fast_available(plan->fast, nb)) {
             SC_CUDA(sc::launch_generic_conv(D, io, nb, 0, D.npix, 0, 0, st));
             ++launches;
         } else {

@@ -205,9 +205,12 @@ def test_edge_geometries_full(sc, path, nside, theta_deg, ntab):
     hemisphere, 2-node tables, theta_max below the pixel spacing: all pixels, sets and values."""
     npix = 12 * nside * nside
     rng = np.random.default_rng(nside * 1000 + ntab)
-    T = rng.standard_normal(ntab)
-    maps = [rng.standard_normal(npix).astype(np.float32)]
     theta = theta_deg * gen.DEG
+    # smooth oscillating kernel: fp32 sensitivity |u K'(u)| comparable to the BASELINE configs (a
+    # white-noise table would amplify the fp32 rounding of the table coordinate beyond 1e-6)
+    _, th = gen.table_nodes(theta, ntab)
+    T = np.exp(-3.0 * (th / theta) ** 2) * np.cos(5.0 * th / theta) + 0.1
+    maps = [rng.standard_normal(npix).astype(np.float32)]
     ref, cnt, sig = O.convolve(nside, T, theta, maps)
     with sc.Plan(nside, T, theta, 1) as plan:
         _set_path(sc, plan, path)
