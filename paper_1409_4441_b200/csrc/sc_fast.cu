@@ -95,7 +95,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     const int N = P.nside;
     const int Lmax = F.Lmax;
 
-    for (int i = tid; i < F.ntab_s; i += NT) tab[i] = P.tab[i];
+    for (int i = tid; i < F.ntab_s; i += NT) tab[i] = P.tabh[i];
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);
     const unsigned zero_bits = kMagicBits + (unsigned)(P.ntab - 1);
     const float tmax = P.tmax, eps = P.eps;

@@ -25,6 +25,9 @@ struct Dev {
     const int *rlo, *rhi;                 // candidate input-ring interval (1-based, inclusive)
     // device interpolation table: K(t) = tab[i].x + t * tab[i].y for t in [i, i+1), t = (1-dot)*scale
     const float2 *tab;
+    // same cells for the half-cell-shifted coordinate t' = t - 1/2 (fast kernel: round(t') = floor(t)):
+    // K(t) = tabh[i].x + t' * tabh[i].y
+    const float2 *tabh;
     // knife-edge overrides decided on the host, sorted by key = p * npix + q
     const unsigned long long *ke_key;
     const unsigned char *ke_in;

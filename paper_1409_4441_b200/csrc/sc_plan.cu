@@ -258,13 +258,14 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
         // device table in the reversed coordinate t = (1 - x) (n-1)/(1-c): node j of the device
         // table is caller node n-1-j.  Cell [j, j+1): K = a_j + t b_j with b_j = T'_{j+1} - T'_j,
         // a_j = T'_j - j b_j  (fp64, rounded once).  Zero padding after the last cell.
-        std::vector<float2> tab((size_t)n_table - 1 + sc::kTabPad);
+        std::vector<float2> tab((size_t)n_table - 1 + sc::kTabPad), tabh(tab.size());
         for (int j = 0; j < n_table - 1; ++j) {
             const double t0 = ktable[n_table - 1 - j], t1 = ktable[n_table - 2 - j];
             const double b = t1 - t0, a = t0 - (double)j * b;
             tab[j] = make_float2((float)a, (float)b);
+            tabh[j] = make_float2((float)(a + 0.5 * b), (float)b);
         }
-        for (size_t j = (size_t)n_table - 1; j < tab.size(); ++j) tab[j] = make_float2(0.f, 0.f);
+        for (size_t j = (size_t)n_table - 1; j < tab.size(); ++j) tab[j] = tabh[j] = make_float2(0.f, 0.f);
 
         if ((st = upload_owned(pl, z, &D.z)) != SC_OK) break;
         if ((st = upload_owned(pl, s, &D.s)) != SC_OK) break;
@@ -275,6 +276,7 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
         if ((st = upload_owned(pl, rlo, &D.rlo)) != SC_OK) break;
         if ((st = upload_owned(pl, rhi, &D.rhi)) != SC_OK) break;
         if ((st = upload_owned(pl, tab, &D.tab)) != SC_OK) break;
+        if ((st = upload_owned(pl, tabh, &D.tabh)) != SC_OK) break;
         D.ke_key = nullptr; D.ke_in = nullptr; D.n_ke = 0;
 
         if ((st = run_audit(pl)) != SC_OK) break;
