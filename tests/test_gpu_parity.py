@@ -254,7 +254,7 @@ def test_batch_chunking_and_host_entry(sc):
 def test_knife_edge_host_adjudication(sc, monkeypatch):
     """Widen the knife-edge band so that many pairs are decided on the host with the host libm;
     sets must still equal the oracle's and the override list must be in use."""
-    monkeypatch.setenv("SC_KNIFE_EDGE_BAND", "1e-7")
+    monkeypatch.setenv("SC_KNIFE_EDGE_BAND", "1e-3")
     nside, theta = 32, 6.0 * gen.DEG
     npix = 12 * nside * nside
     T = np.ones(16)
