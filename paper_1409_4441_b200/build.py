@@ -12,8 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libsc.so")
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["sc_plan.cu", "sc_generic.cu", "sc_fast.cu"]
-HEADERS = [os.path.join(CSRC, "sc_internal.cuh"), os.path.join(ROOT, "include", "sc.h")]
+SOURCES = ["sc_plan.cu", "sc_generic.cu", "sc_fast.cu", "sc_belt.cu"]
+HEADERS = [os.path.join(CSRC, "sc_internal.cuh"), os.path.join(CSRC, "sc_fast.cuh"), os.path.join(ROOT, "include", "sc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          # fp64 inclusion test is specified without FMA contraction on the host side as well

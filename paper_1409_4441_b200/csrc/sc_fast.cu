@@ -17,37 +17,14 @@
 //  * Inclusion: t < tmax - 1 needs no test at all (fast path); the last cell and everything beyond
 //    takes a branch: t > tmax + eps -> excluded, |t - tmax| <= eps -> canonical fp64 test for each
 //    of the 8 images separately (bit-exact with the oracle), else included.
-#include "sc_internal.cuh"
+#include "sc_fast.cuh"
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <vector>
 
 namespace sc {
-
-constexpr int kMaxThreads = 512;
-constexpr float kMagic = 12582912.0f;             // 1.5 * 2^23: low mantissa bits = round(x)
-constexpr unsigned kMagicBits = 0x4B400000u;
-
-struct PairEnt {            // uniform per (base ring, input ring); 48 bytes
-    float A;                // A * scale - 0.5   (table coordinate shifted by half a cell)
-    float c1, c2, c3;       // B * scale * {1/2, -1/24, 1/720}
-    float dphi;             // azimuthal pixel spacing of the input ring
-    float cdc;              // pi / (4 ip ip')
-    int rq, hw, ipq, shq;   // input ring, half window (pixels), pixels per quadrant, shift flag
-    int start_n, start_s;   // first pixel of the input ring and of its southern mirror
-};
-
-struct FastDev {
-    const PairEnt *pairs;
-    const int *pair_off;    // [nslots + 1]
-    const int4 *tiles;      // (ring, k0, slot, 0)
-    int ntiles;
-    int *counter;
-    int Lmax;               // staged positions per plane
-    int ntab_s;             // entries of the shared-memory table
-    int R;
-};
 
 // floor(Y / d) and remainder for 0 <= Y < 2^31 with M0 = floor((2^32 - 1) / d): one multiply-high
 // and one fix-up instead of an integer division
@@ -257,6 +234,18 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
+struct BeltDev {            // mirrors sc_belt.cu
+    const PairEnt *pairs;
+    const int *pair_off;
+    const int *woff;
+    const int4 *tiles;
+    int ntiles;
+    int *counter;
+    int Lp, pw_max, nbuf;
+};
+cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
+                        cudaStream_t st);
+
 struct FastCfg {            // per batch size
     bool ok = false;
     int threads = 0, R = 1, Lmax = 0;
@@ -273,6 +262,14 @@ struct FastPlan {
     int polar = 0;
     FastCfg cfg[kMaxB + 1];
     int nsm = 148;
+    // belt kernel
+    bool belt_ok = false;
+    BeltDev belt{};
+    int belt_threads = 0;
+    size_t belt_smem = 0;
+    int *woff = nullptr;
+    int4 *belt_tiles = nullptr;
+    int *belt_counter = nullptr;
 };
 
 template <int B, int R>
@@ -283,6 +280,7 @@ static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P
     e = cudaMemsetAsync(fp->counter, 0, sizeof(int), st);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, c.ntiles);
+    if (grid <= 0) return cudaSuccess;
     sym_kernel<B, R><<<grid, c.threads, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
@@ -298,7 +296,12 @@ cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cud
         case 3: e = launch_sym<3, 1>(fp, c, P, io, st); break;
         default: e = launch_sym<4, 1>(fp, c, P, io, st); break;
     }
-    if (e == cudaSuccess) *launches = 1;
+    if (e != cudaSuccess) return e;
+    *launches = c.ntiles > 0 ? 1 : 0;
+    if (fp->belt_ok) {
+        e = launch_belt(P, fp->belt, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
+        if (e == cudaSuccess) ++*launches;
+    }
     return e;
 }
 
@@ -308,6 +311,7 @@ void fast_plan_destroy(FastPlan *fp) {
     if (!fp) return;
     cudaFree(fp->pairs); cudaFree(fp->pair_off); cudaFree(fp->counter);
     for (auto &c : fp->cfg) cudaFree(c.tiles);
+    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->belt_counter);
     delete fp;
 }
 
@@ -399,6 +403,54 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     if ((e = cudaMemcpy(fp->pairs, pairs.data(), pairs.size() * sizeof(PairEnt), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
     if ((e = cudaMemcpy(fp->pair_off, pair_off.data(), pair_off.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
 
+    // ---- belt kernel: base rings whose input rings all have 4N pixels ------------------------------
+    std::vector<char> is_belt(2 * N + 1, 0);
+    const bool no_belt = std::getenv("SC_NO_BELT") != nullptr;
+    if (!no_belt && N % 128 == 0 && N >= 512) {
+        const int bthreads = std::min(kMaxThreads, N / 4);
+        const int T = 4 * bthreads;
+        std::vector<int> woff(pairs.size(), 0);
+        std::vector<int4> btiles;
+        int pw_max = 0, hw_max = 0;
+        for (int r = 2 * N; r > polar; --r) {
+            if (ipof(r) != N) continue;
+            bool all = true;
+            for (const PairEnt &pe : per_ring[r]) if (pe.ipq != N) { all = false; break; }
+            if (!all) continue;
+            is_belt[r] = 1;
+            int off = 0;
+            const int base = pair_off[slot_of[r]];
+            for (size_t i = 0; i < per_ring[r].size(); ++i) {
+                woff[base + i] = off;
+                off += 6 + 2 * per_ring[r][i].hw + 8;            // kPwPad + 2hw + 8 (sc_belt.cu)
+                hw_max = std::max(hw_max, per_ring[r][i].hw);
+            }
+            pw_max = std::max(pw_max, off);
+            for (int k0 = 0; k0 < N; k0 += T) btiles.push_back(make_int4(r, k0, slot_of[r], 0));
+        }
+        if (!btiles.empty()) {
+            const int Lp = T - 4 + 4 * ((2 * hw_max + 4 + 3 + 3) >> 2);
+            int nbuf = 0;
+            size_t bsmem = 0;
+            for (int nb : {3, 2}) {
+                bsmem = (size_t)nb * 8 * Lp * 4 + (size_t)pw_max * 8;
+                if (bsmem + 2048 <= (size_t)smem_optin) { nbuf = nb; break; }
+            }
+            if (nbuf) {
+                if ((e = cudaMalloc((void **)&fp->woff, woff.size() * sizeof(int))) != cudaSuccess) return fail(e);
+                if ((e = cudaMemcpy(fp->woff, woff.data(), woff.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+                if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
+                if ((e = cudaMemcpy(fp->belt_tiles, btiles.data(), btiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+                if ((e = cudaMalloc((void **)&fp->belt_counter, sizeof(int))) != cudaSuccess) return fail(e);
+                fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, (int)btiles.size(),
+                                   fp->belt_counter, Lp, pw_max, nbuf};
+                fp->belt_threads = bthreads; fp->belt_smem = bsmem; fp->belt_ok = true;
+            } else {
+                std::fill(is_belt.begin(), is_belt.end(), 0);
+            }
+        }
+    }
+
     // per batch size: threads per CTA so that table + double-buffered stage fit in shared memory
     (void)max_batch;
     for (int B = 1; B <= kMaxB; ++B) {
@@ -409,6 +461,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             std::vector<int4> tiles;
             // larger rings first: long tiles start early, ragged small ones fill the tail
             for (int r = 2 * N; r > polar; --r) {
+                if (is_belt[r]) continue;
                 const int ip = ipof(r), sh = shof(r);
                 for (int k0 = 0; k0 < ip; k0 += T) {
                     tiles.push_back(make_int4(r, k0, slot_of[r], 0));
