@@ -7,8 +7,9 @@
 //   A. evaluates the taps W[r'][j] ONCE -- same fp32 geometry, table lookup and inclusion rule as
 //      the sym kernel (uncertain taps are set to 0 and decided per pixel pair in fp64 afterwards) --
 //      and stores them in shared memory as pairs (w[x], w[x-1]);
-//   B. for every input ring stages the runs of the 8 symmetric images (4 quadrants x north/south)
-//      as 8 contiguous planes with TMA bulk copies (cp.async.bulk + mbarrier, double buffered);
+//   B. a dedicated producer warp stages, for every input ring, the runs of the 8 symmetric images
+//      (4 quadrants x north/south) as 8 contiguous planes with TMA bulk copies (cp.async.bulk) into a
+//      ring of NBUF buffers guarded by full/empty mbarriers -- no block-wide barrier per ring;
 //   C. runs the stencil: a thread owns 4 consecutive pixels x 8 images = 32 accumulators, reads
 //      LDS.128 (4 positions of one image, conflict free) and issues packed FFMA2 over pixel pairs:
 //      (acc_k, acc_k+1) += (w[s-k], w[s-k-1]) * m[s].   One FMA per pair: 4 B of shared-memory traffic
@@ -98,6 +99,15 @@ __device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j
     return fmaf(tp, el.y, el.x);
 }
 
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bar_consumers(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
+
+// All warps run the stencil; warp 0 is also the TMA producer: after each ring it consumes it issues
+// the copies of the ring NBUF-1 ahead in the (tile, map, ring) sequence (its own cursor, so it runs
+// across map and tile boundaries).  Warps meet only through the full/empty mbarriers of the NBUF
+// stage buffers: there is no block-wide barrier in the ring loop.
 template <int NBUF>
 __global__ void __launch_bounds__(kMaxThreads, 1)
 belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
@@ -108,28 +118,71 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
     const int Lp = F.Lp;
     float *stage = reinterpret_cast<float *>(smem_raw);                         // [NBUF][8][Lp]
     float2 *pw = reinterpret_cast<float2 *>(smem_raw + (size_t)NBUF * 8 * Lp * 4);   // [pw_max]
-    __shared__ unsigned long long full_bar[NBUF];
-    __shared__ int s_tile, s_nexc;
+    __shared__ unsigned long long full_bar[NBUF], empty_bar[NBUF];
+    __shared__ int s_nexc;
     __shared__ int s_exc_e[kMaxExc], s_exc_j[kMaxExc];
     __shared__ float s_exc_k[kMaxExc];
 
     if (tid == 0) {
-        for (int i = 0; i < NBUF; ++i) mbar_init(&full_bar[i], 1);
+        for (int i = 0; i < NBUF; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], NT / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    unsigned phase_bits = 0;                 // parity of the next completion of full_bar[i] in bit i
+    __syncthreads();
+    unsigned it = 0;                          // rings processed so far: buffer it % NBUF, use it / NBUF
 
-    while (true) {
-        __syncthreads();
-        if (tid == 0) { s_tile = atomicAdd(F.counter, 1); s_nexc = 0; }
-        __syncthreads();
-        const int tile = s_tile;
-        if (tile >= F.ntiles) break;
+    // ---- producer cursor (meaningful in warp 0 only) ----------------------------------------------
+    unsigned pit = 0;                         // rings issued so far
+    int p_tile = blockIdx.x, p_b = 0, p_e = 0, p_e1 = 0, p_r = 0, p_k0 = 0;
+    bool p_valid = false;
+    auto produce = [&]() {                    // issue the TMA copies of the next ring, if any
+        if (!p_valid) {
+            if (p_tile >= F.ntiles) return;
+            const int4 tl = F.tiles[p_tile];
+            p_r = tl.x; p_k0 = tl.y; p_e = F.pair_off[tl.z]; p_e1 = F.pair_off[tl.z + 1]; p_b = 0;
+            p_valid = true;
+        }
+        const int lane = tid & 31;
+        const int buf = pit % NBUF;
+        const unsigned use = pit / NBUF;
+        const int sh = (p_r - N) & 1;
+        const PairEnt pe = F.pairs[p_e];
+        const int delta = (1 - sh + pe.shq) >> 1;
+        const int first_pos = p_k0 + delta - pe.hw;
+        const int w0a = first_pos & ~3;
+        const int len = T - 4 + 4 * ((2 * pe.hw + 4 + (first_pos - w0a) + 3) >> 2);   // floats
+        unsigned long long *bar = &full_bar[buf];
+        mbar_wait(&empty_bar[buf], (use & 1u) ^ 1u);          // every warp has released this buffer
+        if (lane == 0) mbar_expect_tx(bar, (unsigned)(8 * len * 4));
+        __syncwarp();
+        if (lane < 8) {                                       // one plane per lane
+            const float *__restrict__ in = io.in[p_b];
+            const int m = lane & 3;
+            const int base = (lane < 4) ? pe.start_n : pe.start_s;
+            int s0 = (w0a + m * N) % N4; if (s0 < 0) s0 += N4;
+            float *dst = stage + ((size_t)buf * 8 + lane) * Lp;
+            const int first = min(len, N4 - s0);
+            tma_load_1d(dst, in + base + s0, (unsigned)(first * 4), bar);
+            if (first < len) tma_load_1d(dst + first, in + base, (unsigned)((len - first) * 4), bar);
+        }
+        ++pit;
+        if (++p_e == p_e1) {                                  // next map of this tile, or next tile
+            if (++p_b < B) p_e = F.pair_off[F.tiles[p_tile].z];
+            else { p_tile += gridDim.x; p_valid = false; }
+        }
+    };
+    if (tid < 32) for (int i = 0; i < NBUF - 1; ++i) produce();
+
+    // ==================================== consumers ====================================
+    const int lane = tid & 31;
+    for (int tile = blockIdx.x; tile < F.ntiles; tile += gridDim.x) {
         const int4 tl = F.tiles[tile];
         const int r = tl.x, k0 = tl.y;
         const int sh = (r - N) & 1;
         const int e0 = F.pair_off[tl.z], e1 = F.pair_off[tl.z + 1];
 
+        bar_consumers(NT);                    // previous tile completely finished (taps, exception list)
+        if (tid == 0) s_nexc = 0;
+        bar_consumers(NT);
         // ---- A. taps ----------------------------------------------------------------------------
         for (int e = e0; e < e1; ++e) {
             const PairEnt pe = F.pairs[e];
@@ -159,61 +212,30 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 pw[wo + xi] = make_float2(w2[0], w2[1]);
             }
         }
-        __syncthreads();
+        bar_consumers(NT);
         const int nexc = s_nexc;
 
-        // ---- B/C. per map: stage rings with TMA, run the stencil ---------------------------------
+        // ---- C. per map: the stencil over the staged rings ---------------------------------------
         for (int b = 0; b < B; ++b) {
             const float *__restrict__ in = io.in[b];
-            float2 tot01[8], tot23[8];
+            float2 tot01[8], tot23[8], acc01[8], acc23[8];
 #pragma unroll
-            for (int g = 0; g < 8; ++g) { tot01[g] = make_float2(0.f, 0.f); tot23[g] = make_float2(0.f, 0.f); }
-
-            auto issue = [&](int e, int buf) {       // thread 0 only
-                const PairEnt pe = F.pairs[e];
-                const int delta = (1 - sh + pe.shq) >> 1;
-                const int w0a = (k0 + delta - pe.hw) & ~3;
-                const int a0i = (k0 + delta - pe.hw) - w0a;
-                const int len = T - 4 + 4 * ((2 * pe.hw + 4 + a0i + 3) >> 2);         // floats, multiple of 4
-                unsigned long long *bar = &full_bar[buf];
-                // bytes: 8 planes x len floats
-                mbar_expect_tx(bar, (unsigned)(8 * len * 4));
-#pragma unroll
-                for (int g = 0; g < 8; ++g) {
-                    const int m = g & 3;
-                    const int base = (g < 4) ? pe.start_n : pe.start_s;
-                    int s0 = (w0a + m * N) % N4; if (s0 < 0) s0 += N4;
-                    float *dst = stage + ((size_t)buf * 8 + g) * Lp;
-                    const int first = min(len, N4 - s0);
-                    tma_load_1d(dst, in + base + s0, (unsigned)(first * 4), bar);
-                    if (first < len) tma_load_1d(dst + first, in + base, (unsigned)((len - first) * 4), bar);
-                }
-            };
-
-            __syncthreads();                         // nobody still reads the buffers of the previous map
-            if (tid == 0) {
-                fence_proxy_async();
-                for (int la = 0; la < NBUF - 1 && e0 + la < e1; ++la) issue(e0 + la, la);
+            for (int g = 0; g < 8; ++g) {
+                tot01[g] = make_float2(0.f, 0.f); tot23[g] = make_float2(0.f, 0.f);
+                acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
             }
-            float2 acc01[8], acc23[8];
-#pragma unroll
-            for (int g = 0; g < 8; ++g) { acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f); }
             int ntaps = 0;
-            for (int e = e0; e < e1; ++e) {
-                const int buf = (e - e0) % NBUF;
-                // make sure everyone has finished with the buffer that is refilled next
-                __syncthreads();
-                if (tid == 0 && e + NBUF - 1 < e1) { fence_proxy_async(); issue(e + NBUF - 1, (e + NBUF - 1 - e0) % NBUF); }
-                mbar_wait(&full_bar[buf], (phase_bits >> buf) & 1u);
-                phase_bits ^= 1u << buf;
-
+            for (int e = e0; e < e1; ++e, ++it) {
+                const int buf = it % NBUF;
+                const unsigned use = it / NBUF;
                 const PairEnt pe = F.pairs[e];
                 const int delta = (1 - sh + pe.shq) >> 1;
                 const int first_pos = k0 + delta - pe.hw;
                 const int a0 = first_pos - (first_pos & ~3);
                 const int ng = (2 * pe.hw + 4 + a0 + 3) >> 2;
-                const float2 *pwe = pw + F.woff[e] + kPwPad - a0;         // pwe[s] with s = 4 g + i - a0 folded in
+                const float2 *pwe = pw + F.woff[e] + kPwPad - a0;         // pwe[4 g + i] = P[4 g + i - a0]
                 const float *pl = stage + (size_t)buf * 8 * Lp + 4 * tid;
+                mbar_wait(&full_bar[buf], use & 1u);
                 for (int g4 = 0; g4 < ng; ++g4) {
                     // pairs P[x] = (w[x], w[x-1]) for x = 4 g4 - 2 .. 4 g4 + 3 (relative to pwe)
                     float2 pwr[6];
@@ -238,6 +260,9 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                         }
                     }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
+                if (tid < 32) produce();                                // keep NBUF-1 rings in flight
                 ntaps += 2 * pe.hw + 1;
                 if (ntaps >= 48 || e + 1 == e1) {
 #pragma unroll
@@ -316,8 +341,6 @@ cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, i
         e = cudaFuncSetAttribute(belt_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    e = cudaMemsetAsync(F.counter, 0, sizeof(int), st);
-    if (e != cudaSuccess) return e;
     const int grid = F.ntiles < nsm ? F.ntiles : nsm;
     if (F.nbuf == 3) belt_kernel<3><<<grid, threads, smem, st>>>(P, F, io, B);
     else belt_kernel<2><<<grid, threads, smem, st>>>(P, F, io, B);
