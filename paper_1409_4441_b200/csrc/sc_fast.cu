@@ -22,6 +22,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdlib>
+#include <cstring>
 #include <vector>
 
 namespace sc {
@@ -60,172 +61,241 @@ static __device__ __noinline__ unsigned sym_exact_mask(const Dev &P, int r, int 
     return mask;
 }
 
-template <int B, int R>
-__global__ void __launch_bounds__(kMaxThreads, 1)
+// Shared-memory slot of staged position i.  A thread owns R adjacent base pixels, so the lanes of a warp
+// read positions R apart: one float4 of padding after every 8 positions makes a stride of 2 or 4
+// positions hit 8 different 16-byte bank groups per quarter warp (stride 1 needs no padding).
+template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) { return R == 1 ? i : i + (i >> 3); }
+
+// Packed fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a; a scalar operand is broadcast by the hardware).
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+
+template <int B, int R, int NTMAX>
+__global__ void __launch_bounds__(NTMAX, 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
+    static_assert(R == 1 || R == 2 || R == 4, "R");
+    constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);
     float4 *stage = reinterpret_cast<float4 *>(smem_raw + (((size_t)F.ntab_s * 8 + 15) & ~(size_t)15));
     __shared__ int s_tile;
+    __shared__ SymTile s_tl;
     const int tid = threadIdx.x, NT = blockDim.x;
-    const int T = NT * R;
+    const int warp = tid >> 5, lane = tid & 31;
     const int N = P.nside;
-    const int Lmax = F.Lmax;
+    const int Ltot = F.Ltot;
 
     for (int i = tid; i < F.ntab_s; i += NT) tab[i] = P.tabh[i];
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);
     const unsigned zero_bits = kMagicBits + (unsigned)(P.ntab - 1);
     const float tmax = P.tmax, eps = P.eps;
+    // shared-memory byte address of tab[0] minus 8 kMagicBits (mod 2^32): tab[bits - kMagicBits] = [tab_sh + 8 bits]
+    const unsigned tab_sh = (unsigned)__cvta_generic_to_shared(tab) - kMagicBits * 8u;
 
     while (true) {
-        __syncthreads();
+        __syncthreads();                               // previous tile finished: stage buffers and s_tl are free
         if (tid == 0) s_tile = atomicAdd(F.counter, 1);
         __syncthreads();
         const int tile = s_tile;
         if (tile >= F.ntiles) break;
-        const int4 tl = F.tiles[tile];
-        const int r = tl.x, k0 = tl.y;
-        const int ip = P.npr[r - 1] >> 2;
+        if (tid < (int)(sizeof(SymTile) / 4))
+            reinterpret_cast<int *>(&s_tl)[tid] = __ldg(reinterpret_cast<const int *>(F.tiles + tile) + tid);
+        __syncthreads();
+        const int nsub = s_tl.nsub, nsteps = s_tl.nsteps;
+        int si = 0;
+        for (int s = 1; s < nsub; ++s) if (warp >= s_tl.sub[s].w0) si = s;
+        const SubTile me = s_tl.sub[si];
+        const bool active = warp < me.w0 + me.nw;
+
+        const int r = me.r, k0 = me.k0;
+        const int ip = r < N ? r : N;                  // base rings are rings 1 .. 2N
         const int ip2 = 2 * ip;
         const unsigned M0 = 0xFFFFFFFFu / (unsigned)ip2;
         int rem_unused;
-        const int sh = (r >= N && r <= 3 * N) ? ((r - N) & 1) : 0;
-        const int klast = min(k0 + T, ip) - 1;
-        const int ka = min(k0 + R * tid, klast);
-        const int ap = 2 * ka + 1 - sh, ap0 = 2 * k0 + 1 - sh, apl = 2 * klast + 1 - sh;
-        const int e0 = F.pair_off[tl.z], e1 = F.pair_off[tl.z + 1];
+        const int sh = (r >= N) ? ((r - N) & 1) : 0;
+        const int klast = k0 + me.n - 1;
+        const int kmine = k0 + R * (32 * (warp - me.w0) + lane);
+        const int ka = min(kmine, klast);
+        const int ap = 2 * ka + 1 - sh, ap0 = 2 * k0 + 1 - sh;
 
-        float tot[R][B][8];
+        float2 tot[R][B][4];
 #pragma unroll
         for (int rr = 0; rr < R; ++rr)
 #pragma unroll
             for (int b = 0; b < B; ++b)
 #pragma unroll
-                for (int g = 0; g < 8; ++g) tot[rr][b][g] = 0.f;
+                for (int g = 0; g < 4; ++g) tot[rr][b][g] = f2(0.f);
 
-        // stage the run of input ring entry e into buffer `buf`
-        auto stage_ring = [&](int e, int buf) {
-            const PairEnt pe = F.pairs[e];
-            const int nq = 4 * pe.ipq;
-            const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
-            const int L = div_fast(apl * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) + pe.hw + R - w0;
-            for (int idx = tid; idx < 4 * L; idx += NT) {
-                const int i = idx >> 2, m = idx & 3;
-                int kq = w0 + i + m * pe.ipq + nq;
-                while (kq >= nq) kq -= nq;
+        // stage the runs of input-ring step `step` of every sub-tile into buffer `buf`; returns this
+        // thread's own PairEnt of that step in pe_next
+        PairEnt pe_next = F.pairs[me.e0];
+        auto stage_step = [&](int step, int buf) {
+            for (int s = 0; s < nsub; ++s) {
+                const SubTile st = s_tl.sub[s];
+                if (step >= st.ne) continue;
+                const PairEnt pe = F.pairs[st.e0 + step];
+                if (s == si) pe_next = pe;
+                const int ips = st.r < N ? st.r : N;
+                const int shs = (st.r >= N) ? ((st.r - N) & 1) : 0;
+                const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
+                const int nq = 4 * pe.ipq;
+                const int a0s = 2 * st.k0 + 1 - shs, als = 2 * (st.k0 + st.n - 1) + 1 - shs;
+                const int w0 = div_fast(a0s * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) - pe.hw;
+                const int L = div_fast(als * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) + pe.hw + R - w0;
+                for (int idx = tid; idx < 4 * L; idx += NT) {
+                    const int i = idx >> 2, m = idx & 3;
+                    int kq = w0 + i + m * pe.ipq + nq;
+                    while (kq >= nq) kq -= nq;
+                    const int sl = st.soff + slot_of_pos<R>(i);
 #pragma unroll
-                for (int b = 0; b < B; ++b) {
-                    float *dn = reinterpret_cast<float *>(stage + (size_t)((buf * B + b) * 2 + 0) * Lmax + i) + m;
-                    float *ds = reinterpret_cast<float *>(stage + (size_t)((buf * B + b) * 2 + 1) * Lmax + i) + m;
-                    cp_async4(dn, io.in[b] + pe.start_n + kq);
-                    cp_async4(ds, io.in[b] + pe.start_s + kq);
+                    for (int b = 0; b < B; ++b) {
+                        float *dn = reinterpret_cast<float *>(stage + (size_t)((buf * B + b) * 2 + 0) * Ltot + sl) + m;
+                        float *ds = reinterpret_cast<float *>(stage + (size_t)((buf * B + b) * 2 + 1) * Ltot + sl) + m;
+                        cp_async4(dn, io.in[b] + pe.start_n + kq);
+                        cp_async4(ds, io.in[b] + pe.start_s + kq);
+                    }
                 }
             }
             cp_async_commit();
         };
 
-        stage_ring(e0, 0);
-        for (int e = e0; e < e1; ++e) {
-            const int buf = (e - e0) & 1;
+        stage_step(0, 0);
+        for (int step = 0; step < nsteps; ++step) {
+            const int buf = step & 1;
+            const PairEnt pe = pe_next;                // own entry of `step` (loaded when it was staged)
             cp_async_wait_all();
-            __syncthreads();                       // ring e staged by everyone; ring e-1 fully consumed
-            if (e + 1 < e1) stage_ring(e + 1, buf ^ 1);
+            __syncthreads();                           // step staged by everyone; step-1 fully consumed
+            if (step + 1 < nsteps) stage_step(step + 1, buf ^ 1);
+            if (!active || step >= me.ne) continue;
 
-            const PairEnt pe = F.pairs[e];
             const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
             int rem;
             const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
-            float dc[R];
-            dc[0] = (float)(ip - rem) * pe.cdc;
-            if (R == 2) dc[R - 1] = (float)(ip - rem + 2 * (ip - pe.ipq)) * pe.cdc - pe.dphi;
+            // azimuth of input pixel kc + j seen from base pixel ka + rr:  d = dcr[rr] + j dphi'
+            float dcr[R];
+#pragma unroll
+            for (int rr = 0; rr < R; ++rr) dcr[rr] = (float)(ip - rem - 2 * rr * pe.ipq) * pe.cdc;
+            // staged position of input pixel kc + j: i0 + j (slot_of_pos: padded against bank conflicts)
+            const int i0 = kc - w0;
             const float4 *pn[B], *ps[B];
 #pragma unroll
             for (int b = 0; b < B; ++b) {
-                pn[b] = stage + (size_t)((buf * B + b) * 2 + 0) * Lmax + (kc - w0);
-                ps[b] = stage + (size_t)((buf * B + b) * 2 + 1) * Lmax + (kc - w0);
+                pn[b] = stage + (size_t)((buf * B + b) * 2 + 0) * Ltot + me.soff;
+                ps[b] = stage + (size_t)((buf * B + b) * 2 + 1) * Ltot + me.soff;
             }
-            float acc[R][B][8];
+            float2 acc[R][B][4];
 #pragma unroll
             for (int rr = 0; rr < R; ++rr)
 #pragma unroll
                 for (int b = 0; b < B; ++b)
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) acc[rr][b][g] = 0.f;
+                    for (int g = 0; g < 4; ++g) acc[rr][b][g] = f2(0.f);
+
+            // last table cell or beyond (rare): exact decision where needed, weight 0 on the common path
+            auto slow = [&](int rr, float tpv, unsigned &bits, int j) {
+                const float t = tpv + 0.5f;
+                if (t >= tmax - eps) {
+                    if (t <= tmax + eps) {                   // decide in fp64, image by image
+                        const unsigned mask = sym_exact_mask(P, r, ka + rr, ip, pe.rq, kc + j, pe.ipq, t);
+                        if (mask) {
+                            const float2 el = tab[P.ntab - 2];
+                            const float Ku = fmaf(fminf(t, tmax) - 0.5f, el.y, el.x);
+#pragma unroll
+                            for (int b = 0; b < B; ++b) {
+                                const int sl = slot_of_pos<R>(i0 + j);
+                                const float4 mn = pn[b][sl], ms = ps[b][sl];
+                                const float mv[8] = {mn.x, mn.y, mn.z, mn.w, ms.x, ms.y, ms.z, ms.w};
+#pragma unroll
+                                for (int g = 0; g < 4; ++g) {
+                                    if (mask & (1u << (2 * g))) acc[rr][b][g].x = fmaf(Ku, mv[2 * g], acc[rr][b][g].x);
+                                    if (mask & (2u << (2 * g))) acc[rr][b][g].y = fmaf(Ku, mv[2 * g + 1], acc[rr][b][g].y);
+                                }
+                            }
+                        }
+                    }
+                    bits = zero_bits;
+                }
+            };
 
             const int jend = pe.hw + R - 1;
-            float jf = (float)(-pe.hw);
-            for (int j = -pe.hw; j <= jend; ++j, jf += 1.0f) {
+            const float2 dphi2 = f2(pe.dphi), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
+            float2 dc2[RP];
+#pragma unroll
+            for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
+            float2 jf = f2((float)(-pe.hw));
+#pragma unroll 2
+            for (int j = -pe.hw; j <= jend; ++j) {
+                float tp[2 * RP];
+                unsigned bits[2 * RP];
+#pragma unroll
+                for (int h = 0; h < RP; ++h) {
+                    const float2 d = __ffma2_rn(jf, dphi2, dc2[h]);
+                    const float2 y = __fmul2_rn(d, d);
+                    float2 p = __ffma2_rn(y, c3, c2);
+                    p = __ffma2_rn(y, p, c1);
+                    const float2 t2 = __ffma2_rn(y, p, A2);          // t - 0.5
+                    const float2 bb = __fadd2_rn(t2, f2(kMagic));
+                    tp[2 * h] = t2.x; tp[2 * h + 1] = t2.y;
+                    bits[2 * h] = __float_as_uint(bb.x); bits[2 * h + 1] = __float_as_uint(bb.y);
+                }
+                unsigned mx = bits[0];
+#pragma unroll
+                for (int rr = 1; rr < R; ++rr) mx = max(mx, bits[rr]);
+                if (mx >= thresh) {
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr)
+                        if (bits[rr] >= thresh) slow(rr, tp[rr], bits[rr], j);
+                }
                 float K[R];
 #pragma unroll
                 for (int rr = 0; rr < R; ++rr) {
-                    const float d = fmaf(jf, pe.dphi, dc[rr]);
-                    const float y = d * d;
-                    float h = fmaf(y, pe.c3, pe.c2);
-                    h = fmaf(y, h, pe.c1);
-                    const float tp = fmaf(y, h, pe.A);          // t - 0.5
-                    unsigned bits = __float_as_uint(tp + kMagic);
-                    if (bits >= thresh) {                        // last table cell or beyond
-                        const float t = tp + 0.5f;
-                        if (t >= tmax - eps) {
-                            if (t <= tmax + eps) {               // decide in fp64, image by image
-                                const unsigned mask = sym_exact_mask(P, r, ka + rr, ip, pe.rq, kc + j, pe.ipq, t);
-                                if (mask) {
-                                    const float2 el = tab[P.ntab - 2];
-                                    const float Ku = fmaf(fminf(t, tmax) - 0.5f, el.y, el.x);
-#pragma unroll
-                                    for (int b = 0; b < B; ++b) {
-                                        const float4 mn = pn[b][j], ms = ps[b][j];
-                                        const float mv[8] = {mn.x, mn.y, mn.z, mn.w, ms.x, ms.y, ms.z, ms.w};
-#pragma unroll
-                                        for (int g = 0; g < 8; ++g)
-                                            if (mask & (1u << g)) acc[rr][b][g] = fmaf(Ku, mv[g], acc[rr][b][g]);
-                                    }
-                                }
-                            }
-                            bits = zero_bits;                    // K = 0 on the common path
-                        }
-                    }
-                    const float2 el = tab[bits - kMagicBits];
-                    K[rr] = fmaf(tp, el.y, el.x);
+                    float2 el;                                  // tab[bits - kMagicBits], one LEA for the address
+                    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + bits[rr] * 8u));
+                    K[rr] = fmaf(tp[rr], el.y, el.x);
                 }
+                const int sl = slot_of_pos<R>(i0 + j);
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
-                    const float4 mn = pn[b][j], ms = ps[b][j];
+                    const float4 mn = pn[b][sl], ms = ps[b][sl];
+                    const float2 m01 = f2(mn.x, mn.y), m23 = f2(mn.z, mn.w), m45 = f2(ms.x, ms.y), m67 = f2(ms.z, ms.w);
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) {
-                        acc[rr][b][0] = fmaf(K[rr], mn.x, acc[rr][b][0]);
-                        acc[rr][b][1] = fmaf(K[rr], mn.y, acc[rr][b][1]);
-                        acc[rr][b][2] = fmaf(K[rr], mn.z, acc[rr][b][2]);
-                        acc[rr][b][3] = fmaf(K[rr], mn.w, acc[rr][b][3]);
-                        acc[rr][b][4] = fmaf(K[rr], ms.x, acc[rr][b][4]);
-                        acc[rr][b][5] = fmaf(K[rr], ms.y, acc[rr][b][5]);
-                        acc[rr][b][6] = fmaf(K[rr], ms.z, acc[rr][b][6]);
-                        acc[rr][b][7] = fmaf(K[rr], ms.w, acc[rr][b][7]);
+                        const float2 Kd = f2(K[rr]);
+                        acc[rr][b][0] = __ffma2_rn(Kd, m01, acc[rr][b][0]);
+                        acc[rr][b][1] = __ffma2_rn(Kd, m23, acc[rr][b][1]);
+                        acc[rr][b][2] = __ffma2_rn(Kd, m45, acc[rr][b][2]);
+                        acc[rr][b][3] = __ffma2_rn(Kd, m67, acc[rr][b][3]);
                     }
                 }
+                jf = __fadd2_rn(jf, f2(1.0f));
             }
 #pragma unroll
             for (int rr = 0; rr < R; ++rr)
 #pragma unroll
                 for (int b = 0; b < B; ++b)
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) tot[rr][b][g] += acc[rr][b][g];
+                    for (int g = 0; g < 4; ++g) tot[rr][b][g] = __fadd2_rn(tot[rr][b][g], acc[rr][b][g]);
         }
 
         // store the 8 images of every valid base pixel
-        const int start_n = P.start[r - 1], start_s = P.start[4 * N - r - 1];
-        const bool south = (r != 2 * N);
+        if (active) {
+            const int start_n = P.start[r - 1], start_s = P.start[4 * N - r - 1];
+            const bool south = (r != 2 * N);
 #pragma unroll
-        for (int rr = 0; rr < R; ++rr) {
-            const int k = k0 + R * tid + rr;
-            if (k <= klast) {
+            for (int rr = 0; rr < R; ++rr) {
+                const int k = kmine + rr;
+                if (k <= klast) {
 #pragma unroll
-                for (int b = 0; b < B; ++b)
+                    for (int b = 0; b < B; ++b) {
+                        const float v[8] = {tot[rr][b][0].x, tot[rr][b][0].y, tot[rr][b][1].x, tot[rr][b][1].y,
+                                            tot[rr][b][2].x, tot[rr][b][2].y, tot[rr][b][3].x, tot[rr][b][3].y};
 #pragma unroll
-                    for (int m = 0; m < 4; ++m) {
-                        io.out[b][start_n + k + m * ip] = tot[rr][b][m] * P.omega;
-                        if (south) io.out[b][start_s + k + m * ip] = tot[rr][b][4 + m] * P.omega;
+                        for (int m = 0; m < 4; ++m) {
+                            io.out[b][start_n + k + m * ip] = v[m] * P.omega;
+                            if (south) io.out[b][start_s + k + m * ip] = v[4 + m] * P.omega;
+                        }
                     }
+                }
             }
         }
     }
@@ -248,15 +318,14 @@ cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, i
 
 struct FastCfg {            // per batch size
     bool ok = false;
-    int threads = 0, R = 1, Lmax = 0;
+    int threads = 0, R = 1, Ltot = 0;
     size_t smem = 0;
-    int4 *tiles = nullptr;
+    SymTile *tiles = nullptr;
     int ntiles = 0;
 };
 
 struct FastPlan {
     PairEnt *pairs = nullptr;
-    int *pair_off = nullptr;
     int *counter = nullptr;
     int ntab_s = 0;
     int polar = 0;
@@ -267,21 +336,22 @@ struct FastPlan {
     BeltDev belt{};
     int belt_threads = 0;
     size_t belt_smem = 0;
+    int *pair_off = nullptr;
     int *woff = nullptr;
     int4 *belt_tiles = nullptr;
     int *belt_counter = nullptr;
 };
 
-template <int B, int R>
+template <int B, int R, int NTMAX>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st) {
-    FastDev F{fp->pairs, fp->pair_off, c.tiles, c.ntiles, fp->counter, c.Lmax, fp->ntab_s, R};
-    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+    FastDev F{fp->pairs, c.tiles, c.ntiles, fp->counter, c.Ltot, fp->ntab_s};
+    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NTMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(fp->counter, 0, sizeof(int), st);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, c.ntiles);
     if (grid <= 0) return cudaSuccess;
-    sym_kernel<B, R><<<grid, c.threads, c.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NTMAX><<<grid, c.threads, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
@@ -289,13 +359,16 @@ cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cud
     *launches = 0;
     if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return cudaErrorInvalidValue;
     const FastCfg &c = fp->cfg[B];
-    cudaError_t e;
-    switch (B) {
-        case 1: e = launch_sym<1, 1>(fp, c, P, io, st); break;
-        case 2: e = launch_sym<2, 1>(fp, c, P, io, st); break;
-        case 3: e = launch_sym<3, 1>(fp, c, P, io, st); break;
-        default: e = launch_sym<4, 1>(fp, c, P, io, st); break;
-    }
+    cudaError_t e = cudaErrorInvalidValue;
+    // more than 256 threads per CTA leaves 128 registers per thread, up to 256 threads 255
+#define SC_SYM_CASE(BB, RR)                                                                  \
+    if (B == BB && c.R == RR)                                                                \
+        e = c.threads > 256 ? launch_sym<BB, RR, 512>(fp, c, P, io, st) : launch_sym<BB, RR, 256>(fp, c, P, io, st);
+    SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
+    SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
+    SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
+    SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
+#undef SC_SYM_CASE
     if (e != cudaSuccess) return e;
     *launches = c.ntiles > 0 ? 1 : 0;
     if (fp->belt_ok) {
@@ -315,12 +388,17 @@ void fast_plan_destroy(FastPlan *fp) {
     delete fp;
 }
 
+static int env_int(const char *name, int dflt) {
+    const char *e = std::getenv(name);
+    return e && *e ? std::atoi(e) : dflt;
+}
+
 FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std::vector<double> &s,
                            int max_batch, int *polar_rings, cudaError_t *err) {
     *err = cudaSuccess;
     *polar_rings = 0;
     const int N = P.nside, nr = 4 * N - 1;
-    const int R = 1;
+    constexpr int Rmax = 4;                        // windows are sized for up to 4 base pixels per thread
     int dev = 0, smem_optin = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
@@ -349,8 +427,6 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         const int ip = ipof(r);
         bool ok = true;
         std::vector<PairEnt> &lst = per_ring[r];
-        const int lo = std::max(1, r - (nr)), hi = nr;
-        (void)lo; (void)hi;
         // walk outwards from r in both directions while rings can hold a neighbour
         auto consider = [&](int rq) -> bool {
             double A64 = 1.0 - (z[r - 1] * z[rq - 1] + s[r - 1] * s[rq - 1]);
@@ -362,8 +438,8 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const double dphi = 2.0 * M_PI / (4.0 * ipq);
             const double H = wmax >= 2.0 ? M_PI : 2.0 * std::asin(std::sqrt(0.5 * wmax));
             const double rho1 = std::fabs(1.0 - (double)ipq / ip);
-            const int hw = (int)std::floor(H / dphi + 0.5 + rho1 * (R - 1) + 1e-6);
-            if ((hw + 1 + R) * dphi > dmax) ok = false;
+            const int hw = (int)std::floor(H / dphi + 0.5 + rho1 * (Rmax - 1) + 1e-6);
+            if ((hw + 1 + Rmax) * dphi > dmax) ok = false;
             PairEnt e;
             e.A = (float)(A64 * P.scale - 0.5);
             e.c1 = (float)(Bs / 2.0); e.c2 = (float)(-Bs / 24.0); e.c3 = (float)(Bs / 720.0);
@@ -374,12 +450,11 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             lst.push_back(e);
             return true;
         };
-        std::vector<PairEnt> down;
         for (int rq = r; rq >= 1; --rq) if (!consider(rq)) break;
         std::reverse(lst.begin(), lst.end());
         for (int rq = r + 1; rq <= nr; ++rq) if (!consider(rq)) break;
         // the window of a whole quadrant must not wrap onto itself
-        for (const PairEnt &e : lst) if (e.ipq + 2 * e.hw + 4 >= 4 * e.ipq) ok = false;
+        for (const PairEnt &e : lst) if (e.ipq + 2 * e.hw + 2 * Rmax + 4 >= 4 * e.ipq) ok = false;
         eligible[r] = ok;
     }
     int polar = 0;
@@ -451,34 +526,85 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         }
     }
 
-    // per batch size: threads per CTA so that table + double-buffered stage fit in shared memory
+    // ---- sym kernel: per batch size pick (threads, R) so that table + double-buffered stage fit ------
+    // Tiles are packed from sub-tiles (runs of base pixels on one ring, 32 R pixels per warp): whole
+    // CTA-wide runs first, the ragged remainders of all rings are bin-packed (first fit, decreasing).
     (void)max_batch;
+    struct Cand { int threads, R; };
     for (int B = 1; B <= kMaxB; ++B) {
         FastCfg &c = fp->cfg[B];
-        for (int threads : {512, 384, 256, 192, 128, 64}) {
-            const int T = threads * R;
-            int Lmax = 0;
-            std::vector<int4> tiles;
-            // larger rings first: long tiles start early, ragged small ones fill the tail
+        std::vector<Cand> cands;
+        if (B == 1) cands = {{256, 4}, {512, 2}, {256, 2}, {128, 2}, {64, 2}};
+        else cands = {{256, 2}, {128, 2}, {64, 2}};
+        const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
+        if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && ft % 32 == 0 && ft <= kMaxThreads)
+            cands.insert(cands.begin(), Cand{ft, fr});
+        for (const Cand &cd : cands) {
+            const int R = cd.R, W = cd.threads / 32, C = 32 * R;
+            struct SubH { int r, k0, n, nw; int Lcap; double work; };
+            auto make_sub = [&](int r, int k0, int n) {
+                SubH sb{r, k0, n, (n + C - 1) / C, 0, 0.0};
+                const int ip = ipof(r), sh = shof(r);
+                const int klast = k0 + n - 1;
+                for (const PairEnt &pe : per_ring[r]) {
+                    const int w0 = ((2 * k0 + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) - pe.hw;
+                    const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0;
+                    sb.Lcap = std::max(sb.Lcap, L);
+                    sb.work += (double)(2 * pe.hw + R);
+                }
+                if (R > 1) sb.Lcap = sb.Lcap + (sb.Lcap >> 3) + 1;      // slot_of_pos padding
+                sb.Lcap = (sb.Lcap + 7) & ~7;
+                sb.work *= sb.nw;
+                return sb;
+            };
+            std::vector<std::vector<SubH>> bins;
+            std::vector<SubH> partial;
             for (int r = 2 * N; r > polar; --r) {
                 if (is_belt[r]) continue;
-                const int ip = ipof(r), sh = shof(r);
-                for (int k0 = 0; k0 < ip; k0 += T) {
-                    tiles.push_back(make_int4(r, k0, slot_of[r], 0));
-                    const int klast = std::min(k0 + T, ip) - 1;
-                    for (const PairEnt &pe : per_ring[r]) {
-                        const int w0 = ((2 * k0 + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) - pe.hw;
-                        const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0;
-                        Lmax = std::max(Lmax, L);
-                    }
+                const int ip = ipof(r);
+                int k0 = 0;
+                for (; ip - k0 >= W * C; k0 += W * C) bins.push_back({make_sub(r, k0, W * C)});
+                if (k0 < ip) partial.push_back(make_sub(r, k0, ip - k0));
+            }
+            const size_t nfull = bins.size();
+            std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
+            std::vector<int> used(nfull, W);
+            for (const SubH &sb : partial) {
+                size_t i = nfull;
+                for (; i < bins.size(); ++i) if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub) break;
+                if (i == bins.size()) { bins.emplace_back(); used.push_back(0); }
+                bins[i].push_back(sb); used[i] += sb.nw;
+            }
+            // longest tiles first
+            std::vector<std::pair<double, size_t>> order;
+            int Ltot = 0;
+            for (size_t i = 0; i < bins.size(); ++i) {
+                double w = 0; int L = 0;
+                for (const SubH &sb : bins[i]) { w = std::max(w, sb.work / sb.nw); L += sb.Lcap; }
+                order.push_back({-w, i});
+                Ltot = std::max(Ltot, L);
+            }
+            std::stable_sort(order.begin(), order.end());
+            const size_t smem = tab_bytes + (size_t)2 * B * 2 * Ltot * 16;
+            if (smem + 2048 > (size_t)smem_optin) continue;
+            std::vector<SymTile> tiles(bins.size());
+            for (size_t t = 0; t < order.size(); ++t) {
+                const std::vector<SubH> &bn = bins[order[t].second];
+                SymTile &tl = tiles[t];
+                std::memset(&tl, 0, sizeof(tl));
+                tl.nsub = (int)bn.size();
+                int w0 = 0, soff = 0;
+                for (int i = 0; i < tl.nsub; ++i) {
+                    const SubH &sb = bn[i];
+                    const int slot = slot_of[sb.r];
+                    tl.sub[i] = SubTile{sb.r, sb.k0, sb.n, pair_off[slot], pair_off[slot + 1] - pair_off[slot], w0, sb.nw, soff};
+                    tl.nsteps = std::max(tl.nsteps, tl.sub[i].ne);
+                    w0 += sb.nw; soff += sb.Lcap;
                 }
             }
-            Lmax = (Lmax + 3) & ~3;
-            const size_t smem = tab_bytes + (size_t)2 * B * 2 * Lmax * 16;
-            if (smem + 1024 > (size_t)smem_optin) continue;
-            c.threads = threads; c.R = R; c.Lmax = Lmax; c.smem = smem; c.ntiles = (int)tiles.size();
-            if ((e = cudaMalloc((void **)&c.tiles, tiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
-            if ((e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+            c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = (int)tiles.size();
+            if ((e = cudaMalloc((void **)&c.tiles, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return fail(e);
+            if (!tiles.empty() && (e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             c.ok = true;
             break;
         }

@@ -17,15 +17,28 @@ struct PairEnt {            // uniform per (base ring, input ring); 48 bytes
     int start_n, start_s;   // first pixel of the input ring and of its southern mirror
 };
 
+// A tile of the sym kernel is a set of up to kMaxSub sub-tiles, each a run of base pixels on one ring that
+// is worked on by `nw` consecutive warps (32 R pixels per warp).  Packing several short runs into one
+// tile keeps all warps of the CTA busy on the short rings of the polar caps.
+constexpr int kMaxSub = 4;
+struct SubTile {
+    int r, k0, n;           // base ring, first base pixel, number of base pixels
+    int e0, ne;             // its input rings: pairs[e0 .. e0 + ne)
+    int w0, nw;             // first warp, number of warps
+    int soff;               // offset (positions) of its staged runs within a stage plane
+};
+struct SymTile {
+    int nsub, nsteps, pad0, pad1;   // nsteps = max ne over the sub-tiles
+    SubTile sub[kMaxSub];
+};
+
 struct FastDev {
     const PairEnt *pairs;
-    const int *pair_off;    // [nslots + 1]
-    const int4 *tiles;      // (ring, k0, slot, 0)
+    const SymTile *tiles;
     int ntiles;
     int *counter;
-    int Lmax;               // staged positions per plane
+    int Ltot;               // staged positions per plane
     int ntab_s;             // entries of the shared-memory table
-    int R;
 };
 
 }  // namespace sc

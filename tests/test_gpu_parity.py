@@ -246,8 +246,11 @@ def test_batch_chunking_and_host_entry(sc):
         host = plan.convolve_host(maps)
     ref, _, _ = O.convolve(cfg.nside, T, cfg.theta_max, maps)
     for b in range(6):
-        np.testing.assert_array_equal(batch[b], single[b])
-        np.testing.assert_array_equal(host[b], single[b])
+        # the host entry runs the same launches as the device entry: bit-identical; a batched launch
+        # may use another pixels-per-thread shape than a single-map launch (different fp32 summation
+        # order), so batch vs single is held to the oracle bar instead
+        np.testing.assert_array_equal(host[b], batch[b])
+        _check_values(batch[b], single[b].astype(np.float64), f"batch6 vs single map{b}")
         _check_values(batch[b], ref[b], f"batch6 map{b}")
 
 
