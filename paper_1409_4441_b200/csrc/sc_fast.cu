@@ -36,13 +36,6 @@ __device__ __forceinline__ int div_fast(int Y, int d, unsigned M0, int &rem) {
     return q;
 }
 
-__device__ __forceinline__ void cp_async4(void *smem_dst, const void *gsrc) {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
 // Exact decisions for the 8 images of one uncertain pair: bit g = 4 h + m set <=> image included.
 static __device__ __noinline__ unsigned sym_exact_mask(const Dev &P, int r, int k, int ip, int rq, int kq,
                                                        int ipq, float t) {
@@ -70,48 +63,122 @@ template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) { re
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
 
-template <int B, int R, int NTMAX>
-__global__ void __launch_bounds__(NTMAX, 1)
+constexpr int kSymProd = 128;     // producer threads per CTA (one warpgroup): they only issue cp.async
+constexpr int kSymBuf = 2;        // stage buffers
+
+// Tile n of this CTA: rows of gridDim.x tiles, alternate rows reversed ("snake") so that the CTAs
+// get equal shares of the work-sorted tile list without a global counter.
+__device__ __forceinline__ int snake_tile(int row, int G, int bid) { return row * G + ((row & 1) ? G - 1 - bid : bid); }
+
+__device__ __forceinline__ float4 lds128(unsigned a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+
+// Warp-specialised: the first blockDim.x - kSymProd threads are consumers (pair loop), the last
+// kSymProd threads are producers (staging).  They meet only through the full/empty mbarriers of the
+// kSymBuf stage buffers; there is no block-wide barrier after the prologue.
+template <int B, int R, int NC>
+__global__ void __launch_bounds__(NC + kSymProd, 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(R == 1 || R == 2 || R == 4, "R");
     constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);
-    float4 *stage = reinterpret_cast<float4 *>(smem_raw + (((size_t)F.ntab_s * 8 + 15) & ~(size_t)15));
-    __shared__ int s_tile;
-    __shared__ SymTile s_tl;
-    const int tid = threadIdx.x, NT = blockDim.x;
-    const int warp = tid >> 5, lane = tid & 31;
+    const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 15) & ~(size_t)15));
+    __shared__ unsigned long long full_bar[kSymBuf], empty_bar[kSymBuf];
+    const int tid = threadIdx.x;
     const int N = P.nside;
     const int Ltot = F.Ltot;
+    const int G = gridDim.x, bid = blockIdx.x;
+    const int nrows = (F.ntiles + G - 1) / G;
 
-    for (int i = tid; i < F.ntab_s; i += NT) tab[i] = P.tabh[i];
-    const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);
-    const unsigned zero_bits = kMagicBits + (unsigned)(P.ntab - 1);
+    for (int i = tid; i < F.ntab_s; i += blockDim.x) tab[i] = P.tabh[i];
+    if (tid == 0) {
+        for (int i = 0; i < kSymBuf; ++i) { mbar_init(&full_bar[i], kSymProd); mbar_init(&empty_bar[i], NC / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    unsigned it = 0;                                     // steps so far: buffer it % kSymBuf, use it / kSymBuf
+    int rem_unused;
+
+    // register budget: the launch gives every thread 65536 / (NC + 128) registers (rounded down to a
+    // multiple of 8); the producer warpgroup hands most of its share to the consumer warpgroups
+    if (tid >= NC) {
+        // ======================================= producers =======================================
+        if (NC == 256) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        const int pt = tid - NC;
+        const int m = pt & 3;                            // quadrant image staged by this thread
+        for (int row = 0; row < nrows; ++row) {
+            const int tile = snake_tile(row, G, bid);
+            if (tile >= F.ntiles) continue;
+            const SymTile *tl = F.tiles + tile;
+            const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
+            for (int step = 0; step < nsteps; ++step, ++it) {
+                const int buf = it % kSymBuf;
+                mbar_wait(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);      // every consumer warp released it
+                for (int s = 0; s < nsub; ++s) {
+                    const int ne = __ldg(&tl->sub[s].ne);
+                    if (step >= ne) continue;
+                    const int r = __ldg(&tl->sub[s].r), k0 = __ldg(&tl->sub[s].k0), n = __ldg(&tl->sub[s].n);
+                    const int soff = __ldg(&tl->sub[s].soff);
+                    const PairEnt pe = F.pairs[__ldg(&tl->sub[s].e0) + step];
+                    const int ips = r < N ? r : N;
+                    const int shs = (r >= N) ? ((r - N) & 1) : 0;
+                    const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
+                    const int nq = 4 * pe.ipq;
+                    const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
+                    const int w0 = div_fast(a0s * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) - pe.hw;
+                    const int L = div_fast(als * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) + pe.hw + R - w0;
+                    int kq0 = w0 + m * pe.ipq + nq;      // in [0, 2 nq)
+                    if (kq0 >= nq) kq0 -= nq;
+                    const unsigned d0 = stage_sh + (unsigned)((buf * B * 2) * Ltot + soff) * 16u + 4u * m;
+                    for (int i = pt >> 2; i < L; i += kSymProd / 4) {
+                        int kq = kq0 + i;                // L < nq: one wrap at most
+                        if (kq >= nq) kq -= nq;
+                        const unsigned d = d0 + 16u * (unsigned)slot_of_pos<R>(i);
+#pragma unroll
+                        for (int b = 0; b < B; ++b) {
+                            cp_async4_s(d + (unsigned)(b * 2 * Ltot) * 16u, io.in[b] + pe.start_n + kq);
+                            cp_async4_s(d + (unsigned)((b * 2 + 1) * Ltot) * 16u, io.in[b] + pe.start_s + kq);
+                        }
+                    }
+                }
+                cp_async_mbar_arrive(&full_bar[buf]);   // arrives when this thread's copies have landed
+            }
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        return;
+    }
+
+    // ========================================= consumers =========================================
+    if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+    const int warp = tid >> 5, lane = tid & 31;
+    const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
     const float tmax = P.tmax, eps = P.eps;
     // shared-memory byte address of tab[0] minus 8 kMagicBits (mod 2^32): tab[bits - kMagicBits] = [tab_sh + 8 bits]
-    const unsigned tab_sh = (unsigned)__cvta_generic_to_shared(tab) - kMagicBits * 8u;
+    const unsigned tab_sh = smem_u32(tab) - kMagicBits * 8u;
 
-    while (true) {
-        __syncthreads();                               // previous tile finished: stage buffers and s_tl are free
-        if (tid == 0) s_tile = atomicAdd(F.counter, 1);
-        __syncthreads();
-        const int tile = s_tile;
-        if (tile >= F.ntiles) break;
-        if (tid < (int)(sizeof(SymTile) / 4))
-            reinterpret_cast<int *>(&s_tl)[tid] = __ldg(reinterpret_cast<const int *>(F.tiles + tile) + tid);
-        __syncthreads();
-        const int nsub = s_tl.nsub, nsteps = s_tl.nsteps;
+    for (int row = 0; row < nrows; ++row) {
+        const int tile = snake_tile(row, G, bid);
+        if (tile >= F.ntiles) continue;
+        const SymTile *tl = F.tiles + tile;
+        const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
         int si = 0;
-        for (int s = 1; s < nsub; ++s) if (warp >= s_tl.sub[s].w0) si = s;
-        const SubTile me = s_tl.sub[si];
+        for (int s = 1; s < nsub; ++s) if (warp >= __ldg(&tl->sub[s].w0)) si = s;
+        SubTile me;
+        {
+            const int4 *q = reinterpret_cast<const int4 *>(&tl->sub[si]);
+            const int4 a = __ldg(q), b = __ldg(q + 1);
+            me.r = a.x; me.k0 = a.y; me.n = a.z; me.e0 = a.w; me.ne = b.x; me.w0 = b.y; me.nw = b.z; me.soff = b.w;
+        }
         const bool active = warp < me.w0 + me.nw;
 
         const int r = me.r, k0 = me.k0;
         const int ip = r < N ? r : N;                  // base rings are rings 1 .. 2N
         const int ip2 = 2 * ip;
         const unsigned M0 = 0xFFFFFFFFu / (unsigned)ip2;
-        int rem_unused;
         const int sh = (r >= N) ? ((r - N) & 1) : 0;
         const int klast = k0 + me.n - 1;
         const int kmine = k0 + R * (32 * (warp - me.w0) + lane);
@@ -126,161 +193,131 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 #pragma unroll
                 for (int g = 0; g < 4; ++g) tot[rr][b][g] = f2(0.f);
 
-        // stage the runs of input-ring step `step` of every sub-tile into buffer `buf`; returns this
-        // thread's own PairEnt of that step in pe_next
         PairEnt pe_next = F.pairs[me.e0];
-        auto stage_step = [&](int step, int buf) {
-            for (int s = 0; s < nsub; ++s) {
-                const SubTile st = s_tl.sub[s];
-                if (step >= st.ne) continue;
-                const PairEnt pe = F.pairs[st.e0 + step];
-                if (s == si) pe_next = pe;
-                const int ips = st.r < N ? st.r : N;
-                const int shs = (st.r >= N) ? ((st.r - N) & 1) : 0;
-                const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
-                const int nq = 4 * pe.ipq;
-                const int a0s = 2 * st.k0 + 1 - shs, als = 2 * (st.k0 + st.n - 1) + 1 - shs;
-                const int w0 = div_fast(a0s * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) - pe.hw;
-                const int L = div_fast(als * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) + pe.hw + R - w0;
-                for (int idx = tid; idx < 4 * L; idx += NT) {
-                    const int i = idx >> 2, m = idx & 3;
-                    int kq = w0 + i + m * pe.ipq + nq;
-                    while (kq >= nq) kq -= nq;
-                    const int sl = st.soff + slot_of_pos<R>(i);
+        for (int step = 0; step < nsteps; ++step, ++it) {
+            const int buf = it % kSymBuf;
+            const PairEnt pe = pe_next;
+            if (step + 1 < me.ne) pe_next = F.pairs[me.e0 + step + 1];       // prefetch under the pair loop
+            mbar_wait(&full_bar[buf], (it / kSymBuf) & 1u);
+            if (active && step < me.ne) {
+                const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
+                int rem;
+                const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
+                // azimuth of input pixel kc + j seen from base pixel ka + rr:  d = dcr[rr] + j dphi'
+                float dcr[R];
 #pragma unroll
-                    for (int b = 0; b < B; ++b) {
-                        float *dn = reinterpret_cast<float *>(stage + (size_t)((buf * B + b) * 2 + 0) * Ltot + sl) + m;
-                        float *ds = reinterpret_cast<float *>(stage + (size_t)((buf * B + b) * 2 + 1) * Ltot + sl) + m;
-                        cp_async4(dn, io.in[b] + pe.start_n + kq);
-                        cp_async4(ds, io.in[b] + pe.start_s + kq);
-                    }
-                }
-            }
-            cp_async_commit();
-        };
+                for (int rr = 0; rr < R; ++rr) dcr[rr] = (float)(ip - rem - 2 * rr * pe.ipq) * pe.cdc;
+                // staged position of input pixel kc + j: i0 + j (slot_of_pos: padded against bank conflicts)
+                const int i0 = kc - w0;
+                unsigned pn[B];                          // shared address of this sub-tile's north plane, map b
+#pragma unroll
+                for (int b = 0; b < B; ++b) pn[b] = stage_sh + (unsigned)(((buf * B + b) * 2) * Ltot + me.soff) * 16u;
+                const unsigned south = (unsigned)Ltot * 16u;
+                float2 acc[R][B][4];
+#pragma unroll
+                for (int rr = 0; rr < R; ++rr)
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) acc[rr][b][g] = f2(0.f);
 
-        stage_step(0, 0);
-        for (int step = 0; step < nsteps; ++step) {
-            const int buf = step & 1;
-            const PairEnt pe = pe_next;                // own entry of `step` (loaded when it was staged)
-            cp_async_wait_all();
-            __syncthreads();                           // step staged by everyone; step-1 fully consumed
-            if (step + 1 < nsteps) stage_step(step + 1, buf ^ 1);
-            if (!active || step >= me.ne) continue;
-
-            const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
-            int rem;
-            const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
-            // azimuth of input pixel kc + j seen from base pixel ka + rr:  d = dcr[rr] + j dphi'
-            float dcr[R];
+                // last table cell or the zero cell after it (rare): exact decision where needed
+                auto slow = [&](int rr, float tpv, unsigned &cb, int pos) {
+                    const float t = tpv + 0.5f;
+                    if (t >= tmax - eps) {
+                        if (t <= tmax + eps) {                   // decide in fp64, image by image
+                            const unsigned mask = sym_exact_mask(P, r, ka + rr, ip, pe.rq, kc + pos - i0, pe.ipq, t);
+                            if (mask) {
+                                const float2 el = tab[P.ntab - 2];
+                                const float Ku = fmaf(fminf(t, tmax) - 0.5f, el.y, el.x);
 #pragma unroll
-            for (int rr = 0; rr < R; ++rr) dcr[rr] = (float)(ip - rem - 2 * rr * pe.ipq) * pe.cdc;
-            // staged position of input pixel kc + j: i0 + j (slot_of_pos: padded against bank conflicts)
-            const int i0 = kc - w0;
-            const float4 *pn[B], *ps[B];
+                                for (int b = 0; b < B; ++b) {
+                                    const unsigned a = pn[b] + 16u * (unsigned)slot_of_pos<R>(pos);
+                                    const float4 mn = lds128(a), ms = lds128(a + south);
+                                    const float mv[8] = {mn.x, mn.y, mn.z, mn.w, ms.x, ms.y, ms.z, ms.w};
 #pragma unroll
-            for (int b = 0; b < B; ++b) {
-                pn[b] = stage + (size_t)((buf * B + b) * 2 + 0) * Ltot + me.soff;
-                ps[b] = stage + (size_t)((buf * B + b) * 2 + 1) * Ltot + me.soff;
-            }
-            float2 acc[R][B][4];
-#pragma unroll
-            for (int rr = 0; rr < R; ++rr)
-#pragma unroll
-                for (int b = 0; b < B; ++b)
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) acc[rr][b][g] = f2(0.f);
-
-            // last table cell or beyond (rare): exact decision where needed, weight 0 on the common path
-            auto slow = [&](int rr, float tpv, unsigned &bits, int j) {
-                const float t = tpv + 0.5f;
-                if (t >= tmax - eps) {
-                    if (t <= tmax + eps) {                   // decide in fp64, image by image
-                        const unsigned mask = sym_exact_mask(P, r, ka + rr, ip, pe.rq, kc + j, pe.ipq, t);
-                        if (mask) {
-                            const float2 el = tab[P.ntab - 2];
-                            const float Ku = fmaf(fminf(t, tmax) - 0.5f, el.y, el.x);
-#pragma unroll
-                            for (int b = 0; b < B; ++b) {
-                                const int sl = slot_of_pos<R>(i0 + j);
-                                const float4 mn = pn[b][sl], ms = ps[b][sl];
-                                const float mv[8] = {mn.x, mn.y, mn.z, mn.w, ms.x, ms.y, ms.z, ms.w};
-#pragma unroll
-                                for (int g = 0; g < 4; ++g) {
-                                    if (mask & (1u << (2 * g))) acc[rr][b][g].x = fmaf(Ku, mv[2 * g], acc[rr][b][g].x);
-                                    if (mask & (2u << (2 * g))) acc[rr][b][g].y = fmaf(Ku, mv[2 * g + 1], acc[rr][b][g].y);
+                                    for (int g = 0; g < 4; ++g) {
+                                        if (mask & (1u << (2 * g))) acc[rr][b][g].x = fmaf(Ku, mv[2 * g], acc[rr][b][g].x);
+                                        if (mask & (2u << (2 * g))) acc[rr][b][g].y = fmaf(Ku, mv[2 * g + 1], acc[rr][b][g].y);
+                                    }
                                 }
                             }
                         }
+                        cb = thresh + 1u;                        // zero cell
                     }
-                    bits = zero_bits;
-                }
-            };
+                };
 
-            const int jend = pe.hw + R - 1;
-            const float2 dphi2 = f2(pe.dphi), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
-            float2 dc2[RP];
+                const float2 dphi2 = f2(pe.dphi), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
+                float2 dc2[RP];
 #pragma unroll
-            for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
-            float2 jf = f2((float)(-pe.hw));
+                for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
+                float2 jf = f2((float)(-pe.hw));
+                const int pend = i0 + pe.hw + R - 1;
 #pragma unroll 2
-            for (int j = -pe.hw; j <= jend; ++j) {
-                float tp[2 * RP];
-                unsigned bits[2 * RP];
+                for (int pos = i0 - pe.hw; pos <= pend; ++pos) {
+                    float tp[2 * RP];
+                    unsigned cb[2 * RP];
 #pragma unroll
-                for (int h = 0; h < RP; ++h) {
-                    const float2 d = __ffma2_rn(jf, dphi2, dc2[h]);
-                    const float2 y = __fmul2_rn(d, d);
-                    float2 p = __ffma2_rn(y, c3, c2);
-                    p = __ffma2_rn(y, p, c1);
-                    const float2 t2 = __ffma2_rn(y, p, A2);          // t - 0.5
-                    const float2 bb = __fadd2_rn(t2, f2(kMagic));
-                    tp[2 * h] = t2.x; tp[2 * h + 1] = t2.y;
-                    bits[2 * h] = __float_as_uint(bb.x); bits[2 * h + 1] = __float_as_uint(bb.y);
-                }
-                unsigned mx = bits[0];
+                    for (int h = 0; h < RP; ++h) {
+                        const float2 d = __ffma2_rn(jf, dphi2, dc2[h]);
+                        const float2 y = __fmul2_rn(d, d);
+                        float2 p = __ffma2_rn(y, c3, c2);
+                        p = __ffma2_rn(y, p, c1);
+                        const float2 t2 = __ffma2_rn(y, p, A2);          // t - 0.5
+                        const float2 bb = __fadd2_rn(t2, f2(kMagic));
+                        tp[2 * h] = t2.x; tp[2 * h + 1] = t2.y;
+                        cb[2 * h] = __float_as_uint(bb.x); cb[2 * h + 1] = __float_as_uint(bb.y);
+                    }
+                    // cells below the last: plain lookup; beyond the zero cell: clamp onto it (weight 0);
+                    // the last cell and the zero cell (t in [tmax - 1, tmax + 1)) take the branch
+                    unsigned mn = cb[0] - thresh;
 #pragma unroll
-                for (int rr = 1; rr < R; ++rr) mx = max(mx, bits[rr]);
-                if (mx >= thresh) {
+                    for (int rr = 1; rr < R; ++rr) mn = min(mn, cb[rr] - thresh);
 #pragma unroll
-                    for (int rr = 0; rr < R; ++rr)
-                        if (bits[rr] >= thresh) slow(rr, tp[rr], bits[rr], j);
-                }
-                float K[R];
+                    for (int rr = 0; rr < R; ++rr) cb[rr] = min(cb[rr], thresh + 1u);
+                    if (mn < 2u) {
 #pragma unroll
-                for (int rr = 0; rr < R; ++rr) {
-                    float2 el;                                  // tab[bits - kMagicBits], one LEA for the address
-                    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + bits[rr] * 8u));
-                    K[rr] = fmaf(tp[rr], el.y, el.x);
-                }
-                const int sl = slot_of_pos<R>(i0 + j);
-#pragma unroll
-                for (int b = 0; b < B; ++b) {
-                    const float4 mn = pn[b][sl], ms = ps[b][sl];
-                    const float2 m01 = f2(mn.x, mn.y), m23 = f2(mn.z, mn.w), m45 = f2(ms.x, ms.y), m67 = f2(ms.z, ms.w);
+                        for (int rr = 0; rr < R; ++rr)
+                            if (cb[rr] >= thresh) slow(rr, tp[rr], cb[rr], pos);
+                    }
+                    float K[R];
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) {
-                        const float2 Kd = f2(K[rr]);
-                        acc[rr][b][0] = __ffma2_rn(Kd, m01, acc[rr][b][0]);
-                        acc[rr][b][1] = __ffma2_rn(Kd, m23, acc[rr][b][1]);
-                        acc[rr][b][2] = __ffma2_rn(Kd, m45, acc[rr][b][2]);
-                        acc[rr][b][3] = __ffma2_rn(Kd, m67, acc[rr][b][3]);
+                        float2 el;                                  // tab[cb - kMagicBits], one LEA for the address
+                        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + cb[rr] * 8u));
+                        K[rr] = fmaf(tp[rr], el.y, el.x);
                     }
+                    const unsigned so = 16u * (unsigned)slot_of_pos<R>(pos);
+#pragma unroll
+                    for (int b = 0; b < B; ++b) {
+                        const float4 mn4 = lds128(pn[b] + so), ms4 = lds128(pn[b] + so + south);
+                        const float2 m01 = f2(mn4.x, mn4.y), m23 = f2(mn4.z, mn4.w), m45 = f2(ms4.x, ms4.y), m67 = f2(ms4.z, ms4.w);
+#pragma unroll
+                        for (int rr = 0; rr < R; ++rr) {
+                            const float2 Kd = f2(K[rr]);
+                            acc[rr][b][0] = __ffma2_rn(Kd, m01, acc[rr][b][0]);
+                            acc[rr][b][1] = __ffma2_rn(Kd, m23, acc[rr][b][1]);
+                            acc[rr][b][2] = __ffma2_rn(Kd, m45, acc[rr][b][2]);
+                            acc[rr][b][3] = __ffma2_rn(Kd, m67, acc[rr][b][3]);
+                        }
+                    }
+                    jf = __fadd2_rn(jf, f2(1.0f));
                 }
-                jf = __fadd2_rn(jf, f2(1.0f));
+#pragma unroll
+                for (int rr = 0; rr < R; ++rr)
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int g = 0; g < 4; ++g) tot[rr][b][g] = __fadd2_rn(tot[rr][b][g], acc[rr][b][g]);
             }
-#pragma unroll
-            for (int rr = 0; rr < R; ++rr)
-#pragma unroll
-                for (int b = 0; b < B; ++b)
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) tot[rr][b][g] = __fadd2_rn(tot[rr][b][g], acc[rr][b][g]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[buf]);         // this warp is done with the buffer
         }
 
         // store the 8 images of every valid base pixel
         if (active) {
             const int start_n = P.start[r - 1], start_s = P.start[4 * N - r - 1];
-            const bool south = (r != 2 * N);
+            const bool south_img = (r != 2 * N);
 #pragma unroll
             for (int rr = 0; rr < R; ++rr) {
                 const int k = kmine + rr;
@@ -292,7 +329,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 #pragma unroll
                         for (int m = 0; m < 4; ++m) {
                             io.out[b][start_n + k + m * ip] = v[m] * P.omega;
-                            if (south) io.out[b][start_s + k + m * ip] = v[4 + m] * P.omega;
+                            if (south_img) io.out[b][start_s + k + m * ip] = v[4 + m] * P.omega;
                         }
                     }
                 }
@@ -342,16 +379,14 @@ struct FastPlan {
     int *belt_counter = nullptr;
 };
 
-template <int B, int R, int NTMAX>
+template <int B, int R, int NC>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st) {
     FastDev F{fp->pairs, c.tiles, c.ntiles, fp->counter, c.Ltot, fp->ntab_s};
-    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NTMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(fp->counter, 0, sizeof(int), st);
+    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, c.ntiles);
     if (grid <= 0) return cudaSuccess;
-    sym_kernel<B, R, NTMAX><<<grid, c.threads, c.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
@@ -360,10 +395,11 @@ cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cud
     if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return cudaErrorInvalidValue;
     const FastCfg &c = fp->cfg[B];
     cudaError_t e = cudaErrorInvalidValue;
-    // more than 256 threads per CTA leaves 128 registers per thread, up to 256 threads 255
+    // more than 256 consumer threads per CTA leave 112 registers per thread, up to 256 threads 200
 #define SC_SYM_CASE(BB, RR)                                                                  \
     if (B == BB && c.R == RR)                                                                \
-        e = c.threads > 256 ? launch_sym<BB, RR, 512>(fp, c, P, io, st) : launch_sym<BB, RR, 256>(fp, c, P, io, st);
+        e = c.threads == 256 ? launch_sym<BB, RR, 256>(fp, c, P, io, st)                     \
+                             : launch_sym<BB, RR, 128>(fp, c, P, io, st);
     SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
     SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
     SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
@@ -534,10 +570,10 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     for (int B = 1; B <= kMaxB; ++B) {
         FastCfg &c = fp->cfg[B];
         std::vector<Cand> cands;
-        if (B == 1) cands = {{256, 4}, {512, 2}, {256, 2}, {128, 2}, {64, 2}};
-        else cands = {{256, 2}, {128, 2}, {64, 2}};
+        if (B == 1) cands = {{256, 4}, {256, 2}, {128, 2}};
+        else cands = {{256, 2}, {128, 2}, {128, 1}};
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
-        if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && ft % 32 == 0 && ft <= kMaxThreads)
+        if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256))
             cands.insert(cands.begin(), Cand{ft, fr});
         for (const Cand &cd : cands) {
             const int R = cd.R, W = cd.threads / 32, C = 32 * R;
