@@ -2,36 +2,26 @@
 //
 // In the belt every ring has 4N pixels, so the pair weight K(p, q) depends only on
 // (ring r, ring r', azimuthal offset j): the convolution is a stencil with per-ring-pair taps
-// (SURVEY.md 8f-1).  Per tile (one ring, T = 4 x threads consecutive base pixels of the first
-// quadrant) the kernel
-//   A. evaluates the taps W[r'][j] ONCE -- same fp32 geometry, table lookup and inclusion rule as
-//      the sym kernel (uncertain taps are set to 0 and decided per pixel pair in fp64 afterwards) --
-//      and stores them in shared memory as pairs (w[x], w[x-1]);
-//   B. a dedicated producer warp stages, for every input ring, the runs of the 8 symmetric images
-//      (4 quadrants x north/south) as 8 contiguous planes with TMA bulk copies (cp.async.bulk) into a
-//      ring of NBUF buffers guarded by full/empty mbarriers -- no block-wide barrier per ring;
-//   C. runs the stencil: a thread owns 4 consecutive pixels x 8 images = 32 accumulators, reads
-//      LDS.128 (4 positions of one image, conflict free) and issues packed FFMA2 over pixel pairs:
-//      (acc_k, acc_k+1) += (w[s-k], w[s-k-1]) * m[s].   One FMA per pair: 4 B of shared-memory traffic
-//      per 4 pairs, no geometry in the inner loop.
+// (SURVEY.md 8f-1).  A tile is T = 4 x NC consecutive base pixels of the first quadrant of one ring;
+// its 8 symmetric images (4 quadrants x north/south) share the taps.  The CTA is warp-specialised:
+//   * NC consumer threads run the stencil: a thread owns 4 consecutive pixels x 8 images = 32
+//     accumulators, reads LDS.128 (4 staged positions of one image, conflict free) and issues packed
+//     FFMA2 over pixel pairs: (acc_k, acc_k+1) += (w[s-k], w[s-k-1]) * m[s] -- one FMA per pair, no
+//     geometry in the inner loop;
+//   * one producer warp stages, ring by ring, the runs of the 8 images as 8 contiguous planes with TMA
+//     bulk copies (cp.async.bulk) into a ring of NBUF buffers guarded by full/empty mbarriers;
+//   * three producer warps evaluate the taps W[r'][j] of the NEXT tile -- same fp32 geometry, table
+//     lookup and inclusion rule as the sym kernel (uncertain taps are set to 0 and decided per pixel
+//     pair in fp64 by the consumers afterwards) -- into the other of two tap buffers.
+// There is no block-wide barrier after the prologue.
 #include "sc_fast.cuh"
 
 namespace sc {
 
-constexpr int kPwPad = 6;     // zero pairs in front of every tap array (alignment offset <= 3, pixel offset <= 3)
-constexpr int kMaxExc = 32;   // uncertain taps per tile that can be listed (more -> counted, see below)
-
-struct BeltDev {
-    const PairEnt *pairs;
-    const int *pair_off;
-    const int *woff;          // per pair entry: offset (in float2) of its tap array within the tile's tap buffer
-    const int4 *tiles;        // (ring, k0, slot, 0)
-    int ntiles;
-    int *counter;
-    int Lp;                   // floats per staged plane (multiple of 4)
-    int pw_max;               // float2 entries of the tap buffer
-    int nbuf;                 // stage buffers
-};
+constexpr int kBeltProd = 128;   // producer threads: warp 0 of them issues TMA, warps 1-3 evaluate taps
+constexpr int kTapThreads = 96;
+constexpr int kMaxBuf = 4;
+constexpr int kBeltSlack = 256;  // floats per staged plane beyond the tile: window + alignment
 
 static __device__ __noinline__ unsigned belt_exact_mask(const Dev &P, int r, int k, int rq, int kq) {
     const int N = P.nside, N4 = 4 * N;
@@ -74,120 +64,152 @@ __device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j
     return fmaf(tp, el.y, el.x);
 }
 
-__device__ __forceinline__ void bar_consumers(int n) { asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory"); }
+__device__ __forceinline__ void bar_named(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// All warps run the stencil; warp 0 is also the TMA producer: after each ring it consumes it issues
-// the copies of the ring NBUF-1 ahead in the (tile, map, ring) sequence (its own cursor, so it runs
-// across map and tile boundaries).  Warps meet only through the full/empty mbarriers of the NBUF
-// stage buffers: there is no block-wide barrier in the ring loop.
-template <int NBUF>
-__global__ void __launch_bounds__(kMaxThreads, 1)
+// Window of input ring `pe` for the tile starting at base pixel k0 of a ring with shift flag sh:
+// first staged position is w0a (multiple of 4), the window proper starts a0 positions later and the
+// consumers walk ng chunks of 4 positions.
+__device__ __forceinline__ void belt_window(const PairEnt &pe, int sh, int k0, int &delta, int &w0a, int &a0, int &ng) {
+    delta = (1 - sh + pe.shq) >> 1;
+    const int first_pos = k0 + delta - pe.hw;
+    w0a = first_pos & ~3;
+    a0 = first_pos - w0a;
+    ng = (2 * pe.hw + 4 + a0 + 3) >> 2;
+}
+
+template <int NC>
+__global__ void __launch_bounds__(NC + kBeltProd, 1)
 belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
+    constexpr int T = 4 * NC, LP = T + kBeltSlack;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int tid = threadIdx.x, NT = blockDim.x;
-    const int T = 4 * NT;
+    const int tid = threadIdx.x, lane = tid & 31;
     const int N = P.nside, N4 = 4 * N;
-    const int Lp = F.Lp;
-    float *stage = reinterpret_cast<float *>(smem_raw);                         // [NBUF][8][Lp]
-    float2 *pw = reinterpret_cast<float2 *>(smem_raw + (size_t)NBUF * 8 * Lp * 4);   // [pw_max]
-    __shared__ unsigned long long full_bar[NBUF], empty_bar[NBUF];
-    __shared__ int s_nexc;
-    __shared__ int s_exc_e[kMaxExc], s_exc_j[kMaxExc];
-    __shared__ float s_exc_k[kMaxExc];
+    const int NBUF = F.nbuf, NTB = F.ntb;
+    float *stage = reinterpret_cast<float *>(smem_raw);                           // [NBUF][8][LP]
+    const TapLayout TL(F.pw_max, F.ne_max);
+    unsigned char *tapbase = smem_raw + (size_t)NBUF * 8 * LP * 4;                // [NTB] tap buffers
+    __shared__ unsigned long long full_bar[kMaxBuf], empty_bar[kMaxBuf], tap_full[2], tap_empty[2];
 
     if (tid == 0) {
-        for (int i = 0; i < NBUF; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], NT / 32); }
+        for (int i = 0; i < kMaxBuf; ++i) { mbar_init(&full_bar[i], 1); mbar_init(&empty_bar[i], NC / 32); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&tap_full[i], kTapThreads); mbar_init(&tap_empty[i], NC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    unsigned it = 0;                          // rings processed so far: buffer it % NBUF, use it / NBUF
+    const int G = gridDim.x, bid = blockIdx.x;
+    const int nrows = (F.ntiles + G - 1) / G;
 
-    // ---- producer cursor (meaningful in warp 0 only) ----------------------------------------------
-    unsigned pit = 0;                         // rings issued so far
-    int p_tile = blockIdx.x, p_b = 0, p_e = 0, p_e1 = 0, p_r = 0, p_k0 = 0;
-    bool p_valid = false;
-    auto produce = [&]() {                    // issue the TMA copies of the next ring, if any
-        if (!p_valid) {
-            if (p_tile >= F.ntiles) return;
-            const int4 tl = F.tiles[p_tile];
-            p_r = tl.x; p_k0 = tl.y; p_e = F.pair_off[tl.z]; p_e1 = F.pair_off[tl.z + 1]; p_b = 0;
-            p_valid = true;
-        }
-        const int lane = tid & 31;
-        const int buf = pit % NBUF;
-        const unsigned use = pit / NBUF;
-        const int sh = (p_r - N) & 1;
-        const PairEnt pe = F.pairs[p_e];
-        const int delta = (1 - sh + pe.shq) >> 1;
-        const int first_pos = p_k0 + delta - pe.hw;
-        const int w0a = first_pos & ~3;
-        const int len = T - 4 + 4 * ((2 * pe.hw + 4 + (first_pos - w0a) + 3) >> 2);   // floats
-        unsigned long long *bar = &full_bar[buf];
-        mbar_wait(&empty_bar[buf], (use & 1u) ^ 1u);          // every warp has released this buffer
-        if (lane == 0) mbar_expect_tx(bar, (unsigned)(8 * len * 4));
-        __syncwarp();
-        if (lane < 8) {                                       // one plane per lane
-            const float *__restrict__ in = io.in[p_b];
-            const int m = lane & 3;
-            const int base = (lane < 4) ? pe.start_n : pe.start_s;
-            int s0 = (w0a + m * N) % N4; if (s0 < 0) s0 += N4;
-            float *dst = stage + ((size_t)buf * 8 + lane) * Lp;
-            const int first = min(len, N4 - s0);
-            tma_load_1d(dst, in + base + s0, (unsigned)(first * 4), bar);
-            if (first < len) tma_load_1d(dst + first, in + base, (unsigned)((len - first) * 4), bar);
-        }
-        ++pit;
-        if (++p_e == p_e1) {                                  // next map of this tile, or next tile
-            if (++p_b < B) p_e = F.pair_off[F.tiles[p_tile].z];
-            else { p_tile += gridDim.x; p_valid = false; }
-        }
-    };
-    if (tid < 32) for (int i = 0; i < NBUF - 1; ++i) produce();
-
-    // ==================================== consumers ====================================
-    const int lane = tid & 31;
-    for (int tile = blockIdx.x; tile < F.ntiles; tile += gridDim.x) {
-        const int4 tl = F.tiles[tile];
-        const int r = tl.x, k0 = tl.y;
-        const int sh = (r - N) & 1;
-        const int e0 = F.pair_off[tl.z], e1 = F.pair_off[tl.z + 1];
-
-        bar_consumers(NT);                    // previous tile completely finished (taps, exception list)
-        if (tid == 0) s_nexc = 0;
-        bar_consumers(NT);
-        // ---- A. taps ----------------------------------------------------------------------------
-        for (int e = e0; e < e1; ++e) {
-            const PairEnt pe = F.pairs[e];
-            const int wo = F.woff[e];
-            // nearest pixel of ring rq in azimuth: kc = k + delta, at angle dcc from p.  In the belt
-            // Y = N (2k + 1 - sh + shq), so delta = (1 - sh + shq) >> 1 and the remainder is N or 0.
-            const int Yk = 1 - sh + pe.shq;
-            const float dcc = (float)(N - ((Yk & 1) ? N : 0)) * pe.cdc;
-            const int nx = kPwPad + 2 * pe.hw + 8;               // x = -kPwPad .. 2hw+7
-            for (int xi = tid; xi < nx; xi += NT) {
-                const int x = xi - kPwPad;
-                float w2[2];
-#pragma unroll
-                for (int q = 0; q < 2; ++q) {
-                    const int xx = x - q;
-                    float w = 0.f;
-                    if (xx >= 0 && xx <= 2 * pe.hw) {
-                        bool unc; float Ku;
-                        w = belt_tap(P, pe, xx - pe.hw, dcc, unc, Ku);
-                        if (unc && q == 0) {                              // list every uncertain tap once
-                            const int slot = atomicAdd(&s_nexc, 1);
-                            if (slot < kMaxExc) { s_exc_e[slot] = e; s_exc_j[slot] = xx - pe.hw; s_exc_k[slot] = Ku; }
+    if (tid >= NC) {
+        if (NC == 256) asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+        if (tid < NC + 32) {
+            // ================================ TMA producer warp ================================
+            int buf = 0; unsigned par = 0;
+            for (int row = 0; row < nrows; ++row) {
+                const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
+                if (tile >= F.ntiles) continue;
+                const int4 tl = F.tiles[tile];
+                const int r = tl.x, k0 = tl.y, ne = tl.w;
+                const int sh = (r - N) & 1;
+                const int e0 = F.pair_off[tl.z];
+                for (int b = 0; b < B; ++b) {
+                    const float *__restrict__ in = io.in[b];
+                    for (int e = 0; e < ne; ++e) {
+                        const PairEnt pe = F.pairs[e0 + e];
+                        int delta, w0a, a0, ng;
+                        belt_window(pe, sh, k0, delta, w0a, a0, ng);
+                        const int len = T - 4 + 4 * ng;                       // floats per plane
+                        unsigned long long *bar = &full_bar[buf];
+                        mbar_wait(&empty_bar[buf], par ^ 1u);                 // every consumer warp released it
+                        if (lane == 0) mbar_expect_tx(bar, (unsigned)(8 * len * 4));
+                        __syncwarp();
+                        if (lane < 8) {                                       // one plane per lane
+                            const int m = lane & 3;
+                            const int base = (lane < 4) ? pe.start_n : pe.start_s;
+                            int s0 = (w0a + m * N) % N4; if (s0 < 0) s0 += N4;
+                            float *dst = stage + ((size_t)buf * 8 + lane) * LP;
+                            const int first = min(len, N4 - s0);
+                            tma_load_1d(dst, in + base + s0, (unsigned)(first * 4), bar);
+                            if (first < len) tma_load_1d(dst + first, in + base, (unsigned)((len - first) * 4), bar);
                         }
+                        if (++buf == NBUF) { buf = 0; par ^= 1u; }
                     }
-                    w2[q] = w;
                 }
-                pw[wo + xi] = make_float2(w2[0], w2[1]);
+            }
+        } else {
+            // ================================ tap producer warps ================================
+            const int pt = tid - NC - 32;
+            int tb = 0; unsigned tpar = 0;
+            for (int row = 0; row < nrows; ++row) {
+                const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
+                if (tile >= F.ntiles) continue;
+                const int4 tl = F.tiles[tile];
+                const int r = tl.x, k0 = tl.y, ne = tl.w;
+                const int sh = (r - N) & 1;
+                const int e0 = F.pair_off[tl.z];
+                unsigned char *tbuf = tapbase + (size_t)tb * TL.bytes;
+                float2 *S = reinterpret_cast<float2 *>(tbuf);
+                int4 *desc = reinterpret_cast<int4 *>(tbuf + TL.desc);
+                int *exc_e = reinterpret_cast<int *>(tbuf + TL.exc_e), *exc_j = reinterpret_cast<int *>(tbuf + TL.exc_j);
+                float *exc_k = reinterpret_cast<float *>(tbuf + TL.exc_k);
+                int *nexc = reinterpret_cast<int *>(tbuf + TL.nexc);
+                mbar_wait(&tap_empty[tb], tpar ^ 1u);                         // consumers are done with this buffer
+                if (pt == 0) *nexc = 0;
+                bar_named(1, kTapThreads);
+                for (int e = 0; e < ne; ++e) {
+                    const PairEnt pe = F.pairs[e0 + e];
+                    const int wo = F.woff[e0 + e];
+                    int delta, w0a, a0, ng;
+                    belt_window(pe, sh, k0, delta, w0a, a0, ng);
+                    if (pt == 0) desc[e] = make_int4(ng, wo * 8, 2 * pe.hw + 1, 0);
+                    // nearest pixel of ring rq in azimuth: kc = k + delta, at angle dcc from p.  In the belt
+                    // Y = N (2k + 1 - sh + shq), so delta = (1 - sh + shq) >> 1 and the remainder is N or 0.
+                    const int Yk = 1 - sh + pe.shq;
+                    const float dcc = (float)(N - ((Yk & 1) ? N : 0)) * pe.cdc;
+                    // S[i] = (w[x], w[x-1]), x = i - 2 - a0: chunk g of 4 staged positions uses S[4g .. 4g+5]
+                    const int nS = 4 * ng + 2;
+                    for (int i = pt; i < nS; i += kTapThreads) {
+                        const int x = i - 2 - a0;
+                        float w2[2];
+#pragma unroll
+                        for (int q = 0; q < 2; ++q) {
+                            const int xx = x - q;
+                            float w = 0.f;
+                            if (xx >= 0 && xx <= 2 * pe.hw) {
+                                bool unc; float Ku;
+                                w = belt_tap(P, pe, xx - pe.hw, dcc, unc, Ku);
+                                if (unc && q == 0) {                          // list every uncertain tap once
+                                    const int slot = atomicAdd(nexc, 1);
+                                    if (slot < kMaxExc) { exc_e[slot] = e; exc_j[slot] = xx - pe.hw; exc_k[slot] = Ku; }
+                                }
+                            }
+                            w2[q] = w;
+                        }
+                        S[wo + i] = make_float2(w2[0], w2[1]);
+                    }
+                }
+                mbar_arrive(&tap_full[tb]);
+                if (++tb == NTB) { tb = 0; tpar ^= 1u; }
             }
         }
-        bar_consumers(NT);
-        const int nexc = s_nexc;
+        return;
+    }
 
-        // ---- C. per map: the stencil over the staged rings ---------------------------------------
+    // ==================================== consumers ====================================
+    if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+    int buf = 0; unsigned par = 0;
+    int tb = 0; unsigned tpar = 0;
+    for (int row = 0; row < nrows; ++row) {
+        const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
+        if (tile >= F.ntiles) continue;
+        const int4 tl = F.tiles[tile];
+        const int r = tl.x, k0 = tl.y, ne = tl.w;
+        const int sh = (r - N) & 1;
+        const int e0 = F.pair_off[tl.z];
+        const unsigned char *tbuf = tapbase + (size_t)tb * TL.bytes;
+        const int4 *desc = reinterpret_cast<const int4 *>(tbuf + TL.desc);
+        mbar_wait(&tap_full[tb], tpar);                       // taps of this tile are in place
+        const int nexc = *reinterpret_cast<const int *>(tbuf + TL.nexc);
+
         for (int b = 0; b < B; ++b) {
             const float *__restrict__ in = io.in[b];
             float2 tot01[8], tot23[8], acc01[8], acc23[8];
@@ -197,28 +219,26 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
             }
             int ntaps = 0;
-            for (int e = e0; e < e1; ++e, ++it) {
-                const int buf = it % NBUF;
-                const unsigned use = it / NBUF;
-                const PairEnt pe = F.pairs[e];
-                const int delta = (1 - sh + pe.shq) >> 1;
-                const int first_pos = k0 + delta - pe.hw;
-                const int a0 = first_pos - (first_pos & ~3);
-                const int ng = (2 * pe.hw + 4 + a0 + 3) >> 2;
-                const float2 *pwe = pw + F.woff[e] + kPwPad - a0;         // pwe[4 g + i] = P[4 g + i - a0]
-                const float *pl = stage + (size_t)buf * 8 * Lp + 4 * tid;
-                mbar_wait(&full_bar[buf], use & 1u);
-                for (int g4 = 0; g4 < ng; ++g4) {
-                    // pairs P[x] = (w[x], w[x-1]) for x = 4 g4 - 2 .. 4 g4 + 3 (relative to pwe)
+            for (int e = 0; e < ne; ++e) {
+                const int4 d = desc[e];                                   // (chunks, tap offset in bytes, taps)
+                const float4 *S4 = reinterpret_cast<const float4 *>(tbuf + d.y);   // S4[2 g + i] = S[4 g + 2 i .. + 1]
+                const float *pl = stage + (size_t)buf * 8 * LP + 4 * tid;
+                mbar_wait(&full_bar[buf], par);
+#pragma unroll 1
+                for (int g4 = 0; g4 < d.x; ++g4) {
+                    // pairs (w[x], w[x-1]) of the 6 tap positions this chunk touches
                     float2 pwr[6];
 #pragma unroll
-                    for (int i = 0; i < 6; ++i) pwr[i] = pwe[4 * g4 - 2 + i];
+                    for (int i = 0; i < 3; ++i) {
+                        const float4 v = S4[2 * g4 + i];
+                        pwr[2 * i] = make_float2(v.x, v.y); pwr[2 * i + 1] = make_float2(v.z, v.w);
+                    }
 #pragma unroll
                     for (int half = 0; half < 2; ++half) {
                         float4 mv[4];
 #pragma unroll
                         for (int q = 0; q < 4; ++q)
-                            mv[q] = *reinterpret_cast<const float4 *>(pl + (size_t)(half * 4 + q) * Lp + 4 * g4);
+                            mv[q] = *reinterpret_cast<const float4 *>(pl + (half * 4 + q) * LP + 4 * g4);
 #pragma unroll
                         for (int q = 0; q < 4; ++q) {
                             const int g = half * 4 + q;
@@ -234,13 +254,12 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
-                if (tid < 32) produce();                                // keep NBUF-1 rings in flight
-                ntaps += 2 * pe.hw + 1;
-                if (ntaps >= 48 || e + 1 == e1) {
+                if (++buf == NBUF) { buf = 0; par ^= 1u; }
+                ntaps += d.z;
+                if (ntaps >= 48 || e + 1 == ne) {
 #pragma unroll
                     for (int g = 0; g < 8; ++g) {
-                        tot01[g].x += acc01[g].x; tot01[g].y += acc01[g].y;
-                        tot23[g].x += acc23[g].x; tot23[g].y += acc23[g].y;
+                        tot01[g] = __fadd2_rn(tot01[g], acc01[g]); tot23[g] = __fadd2_rn(tot23[g], acc23[g]);
                         acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
                     }
                     ntaps = 0;
@@ -270,10 +289,12 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     }
                 };
                 if (nexc <= kMaxExc) {
-                    for (int i = 0; i < nexc; ++i) apply(F.pairs[s_exc_e[i]], s_exc_j[i], s_exc_k[i]);
+                    const int *exc_e = reinterpret_cast<const int *>(tbuf + TL.exc_e), *exc_j = reinterpret_cast<const int *>(tbuf + TL.exc_j);
+                    const float *exc_k = reinterpret_cast<const float *>(tbuf + TL.exc_k);
+                    for (int i = 0; i < nexc; ++i) apply(F.pairs[e0 + exc_e[i]], exc_j[i], exc_k[i]);
                 } else {                              // list overflow: rescan every tap (never seen in practice)
-                    for (int e = e0; e < e1; ++e) {
-                        const PairEnt pe = F.pairs[e];
+                    for (int e = 0; e < ne; ++e) {
+                        const PairEnt pe = F.pairs[e0 + e];
                         const int Yk = 1 - sh + pe.shq;
                         const float dcc = (float)(N - ((Yk & 1) ? N : 0)) * pe.cdc;
                         for (int j = -pe.hw; j <= pe.hw; ++j) {
@@ -299,24 +320,32 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 *reinterpret_cast<float4 *>(out + ((g < 4) ? start_n : start_s) + k + (g & 3) * N) = v;
             }
         }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tap_empty[tb]);                       // tap buffer may be refilled
+        if (++tb == NTB) { tb = 0; tpar ^= 1u; }
     }
 }
 
 // host ------------------------------------------------------------------------------------------
+size_t belt_smem_bytes(int NC, int nbuf, int ntb, int pw_max, int ne_max) {
+    return (size_t)nbuf * 8 * (4 * NC + kBeltSlack) * 4 + (size_t)ntb * TapLayout(pw_max, ne_max).bytes;
+}
+int belt_max_chunk_floats() { return kBeltSlack + 4; }                   // 4 ng may not exceed this
+
+template <int NC>
+static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io, int B, size_t smem, int nsm, cudaStream_t st) {
+    cudaError_t e = cudaFuncSetAttribute(belt_kernel<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int grid = F.ntiles < nsm ? F.ntiles : nsm;
+    belt_kernel<NC><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
                         cudaStream_t st) {
-    cudaError_t e;
-    if (F.nbuf == 3) {
-        e = cudaFuncSetAttribute(belt_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-    } else {
-        e = cudaFuncSetAttribute(belt_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-    }
-    const int grid = F.ntiles < nsm ? F.ntiles : nsm;
-    if (F.nbuf == 3) belt_kernel<3><<<grid, threads, smem, st>>>(P, F, io, B);
-    else belt_kernel<2><<<grid, threads, smem, st>>>(P, F, io, B);
-    return cudaGetLastError();
+    if (threads == 256) return launch_belt_nc<256>(P, F, io, B, smem, nsm, st);
+    if (threads == 128) return launch_belt_nc<128>(P, F, io, B, smem, nsm, st);
+    return cudaErrorInvalidValue;
 }
 
 }  // namespace sc

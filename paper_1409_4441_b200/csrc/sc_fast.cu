@@ -341,15 +341,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-struct BeltDev {            // mirrors sc_belt.cu
-    const PairEnt *pairs;
-    const int *pair_off;
-    const int *woff;
-    const int4 *tiles;
-    int ntiles;
-    int *counter;
-    int Lp, pw_max, nbuf;
-};
+size_t belt_smem_bytes(int NC, int nbuf, int ntb, int pw_max, int ne_max);
+int belt_max_chunk_floats();
 cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
                         cudaStream_t st);
 
@@ -376,7 +369,6 @@ struct FastPlan {
     int *pair_off = nullptr;
     int *woff = nullptr;
     int4 *belt_tiles = nullptr;
-    int *belt_counter = nullptr;
 };
 
 template <int B, int R, int NC>
@@ -420,7 +412,7 @@ void fast_plan_destroy(FastPlan *fp) {
     if (!fp) return;
     cudaFree(fp->pairs); cudaFree(fp->pair_off); cudaFree(fp->counter);
     for (auto &c : fp->cfg) cudaFree(c.tiles);
-    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->belt_counter);
+    cudaFree(fp->woff); cudaFree(fp->belt_tiles);
     delete fp;
 }
 
@@ -517,12 +509,13 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     // ---- belt kernel: base rings whose input rings all have 4N pixels ------------------------------
     std::vector<char> is_belt(2 * N + 1, 0);
     const bool no_belt = std::getenv("SC_NO_BELT") != nullptr;
-    if (!no_belt && N % 128 == 0 && N >= 512) {
-        const int bthreads = std::min(kMaxThreads, N / 4);
-        const int T = 4 * bthreads;
+    const int bNC = (N % 1024 == 0) ? 256 : (N % 512 == 0 ? 128 : 0);       // consumer threads, tile = 4 bNC pixels
+    if (!no_belt && bNC) {
+        const int T = 4 * bNC;
         std::vector<int> woff(pairs.size(), 0);
         std::vector<int4> btiles;
-        int pw_max = 0, hw_max = 0;
+        int pw_max = 0, ne_max = 0;
+        bool fits = true;
         for (int r = 2 * N; r > polar; --r) {
             if (ipof(r) != N) continue;
             bool all = true;
@@ -532,33 +525,33 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             int off = 0;
             const int base = pair_off[slot_of[r]];
             for (size_t i = 0; i < per_ring[r].size(); ++i) {
+                const int ng_max = (2 * per_ring[r][i].hw + 4 + 3 + 3) >> 2;   // chunks of 4 staged positions
+                if (4 * ng_max > belt_max_chunk_floats()) fits = false;
                 woff[base + i] = off;
-                off += 6 + 2 * per_ring[r][i].hw + 8;            // kPwPad + 2hw + 8 (sc_belt.cu)
-                hw_max = std::max(hw_max, per_ring[r][i].hw);
+                off += (4 * ng_max + 2 + 1) & ~1;                              // tap pairs, even count
             }
             pw_max = std::max(pw_max, off);
-            for (int k0 = 0; k0 < N; k0 += T) btiles.push_back(make_int4(r, k0, slot_of[r], 0));
+            ne_max = std::max(ne_max, (int)per_ring[r].size());
+            for (int k0 = 0; k0 < N; k0 += T) btiles.push_back(make_int4(r, k0, slot_of[r], (int)per_ring[r].size()));
         }
-        if (!btiles.empty()) {
-            const int Lp = T - 4 + 4 * ((2 * hw_max + 4 + 3 + 3) >> 2);
-            int nbuf = 0;
-            size_t bsmem = 0;
-            for (int nb : {3, 2}) {
-                bsmem = (size_t)nb * 8 * Lp * 4 + (size_t)pw_max * 8;
-                if (bsmem + 2048 <= (size_t)smem_optin) { nbuf = nb; break; }
+        int nbuf = 0, ntb = 0;
+        size_t bsmem = 0;
+        if (fits && !btiles.empty()) {
+            const int combos[6][2] = {{2, 4}, {2, 3}, {1, 4}, {2, 2}, {1, 3}, {1, 2}};       // (tap buffers, stage buffers)
+            for (const auto &cb : combos) {
+                bsmem = belt_smem_bytes(bNC, cb[1], cb[0], pw_max, ne_max);
+                if (bsmem + 2048 <= (size_t)smem_optin) { ntb = cb[0]; nbuf = cb[1]; break; }
             }
-            if (nbuf) {
-                if ((e = cudaMalloc((void **)&fp->woff, woff.size() * sizeof(int))) != cudaSuccess) return fail(e);
-                if ((e = cudaMemcpy(fp->woff, woff.data(), woff.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
-                if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
-                if ((e = cudaMemcpy(fp->belt_tiles, btiles.data(), btiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
-                if ((e = cudaMalloc((void **)&fp->belt_counter, sizeof(int))) != cudaSuccess) return fail(e);
-                fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, (int)btiles.size(),
-                                   fp->belt_counter, Lp, pw_max, nbuf};
-                fp->belt_threads = bthreads; fp->belt_smem = bsmem; fp->belt_ok = true;
-            } else {
-                std::fill(is_belt.begin(), is_belt.end(), 0);
-            }
+        }
+        if (nbuf) {
+            if ((e = cudaMalloc((void **)&fp->woff, woff.size() * sizeof(int))) != cudaSuccess) return fail(e);
+            if ((e = cudaMemcpy(fp->woff, woff.data(), woff.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+            if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
+            if ((e = cudaMemcpy(fp->belt_tiles, btiles.data(), btiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+            fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, (int)btiles.size(), pw_max, ne_max, nbuf, ntb};
+            fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true;
+        } else {
+            std::fill(is_belt.begin(), is_belt.end(), 0);
         }
     }
 

@@ -41,6 +41,33 @@ struct FastDev {
     int ntab_s;             // entries of the shared-memory table
 };
 
+constexpr int kMaxExc = 32;      // uncertain taps per belt tile that can be listed (more -> rescan)
+
+struct BeltDev {
+    const PairEnt *pairs;
+    const int *pair_off;
+    const int *woff;          // per pair entry: offset (in float2, even) of its tap array within a tap buffer
+    const int4 *tiles;        // (ring, k0, slot, number of input rings)
+    int ntiles;
+    int pw_max;               // float2 entries of a tap buffer
+    int ne_max;               // input rings per tile, at most
+    int nbuf;                 // stage buffers
+    int ntb;                  // tap buffers (1 or 2)
+};
+
+// Layout of one tap buffer in shared memory (bytes): taps | ring descriptors | exception list
+struct TapLayout {
+    unsigned desc, exc_e, exc_j, exc_k, nexc, bytes;
+    __host__ __device__ TapLayout(int pw_max, int ne_max) {
+        desc = (unsigned)pw_max * 8u;
+        exc_e = desc + (unsigned)ne_max * 16u;
+        exc_j = exc_e + kMaxExc * 4u;
+        exc_k = exc_j + kMaxExc * 4u;
+        nexc = exc_k + kMaxExc * 4u;
+        bytes = (nexc + 16u + 15u) & ~15u;
+    }
+};
+
 // ---- mbarrier / TMA bulk copy -------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
