@@ -16,6 +16,10 @@
 // There is no block-wide barrier after the prologue.
 #include "sc_fast.cuh"
 
+#ifndef SC_BELT_PREFETCH
+#define SC_BELT_PREFETCH 0
+#endif
+
 namespace sc {
 
 constexpr int kBeltProd = 128;   // producer threads: warp 0 of them issues TMA, warps 1-3 evaluate taps
@@ -113,13 +117,15 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 const int e0 = F.pair_off[tl.z];
                 for (int b = 0; b < B; ++b) {
                     const float *__restrict__ in = io.in[b];
+                    PairEnt pe_next = F.pairs[e0];
                     for (int e = 0; e < ne; ++e) {
-                        const PairEnt pe = F.pairs[e0 + e];
+                        const PairEnt pe = pe_next;
+                        if (e + 1 < ne) pe_next = F.pairs[e0 + e + 1];      // prefetched while waiting below
                         int delta, w0a, a0, ng;
                         belt_window(pe, sh, k0, delta, w0a, a0, ng);
                         const int len = T - 4 + 4 * ng;                       // floats per plane
                         unsigned long long *bar = &full_bar[buf];
-                        mbar_wait(&empty_bar[buf], par ^ 1u);                 // every consumer warp released it
+                        mbar_wait_sleep(&empty_bar[buf], par ^ 1u);           // every consumer warp released it
                         if (lane == 0) mbar_expect_tx(bar, (unsigned)(8 * len * 4));
                         __syncwarp();
                         if (lane < 8) {                                       // one plane per lane
@@ -152,7 +158,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 int *exc_e = reinterpret_cast<int *>(tbuf + TL.exc_e), *exc_j = reinterpret_cast<int *>(tbuf + TL.exc_j);
                 float *exc_k = reinterpret_cast<float *>(tbuf + TL.exc_k);
                 int *nexc = reinterpret_cast<int *>(tbuf + TL.nexc);
-                mbar_wait(&tap_empty[tb], tpar ^ 1u);                         // consumers are done with this buffer
+                mbar_wait_sleep(&tap_empty[tb], tpar ^ 1u);                   // consumers are done with this buffer
                 if (pt == 0) *nexc = 0;
                 bar_named(1, kTapThreads);
                 for (int e = 0; e < ne; ++e) {
@@ -224,34 +230,49 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 const float4 *S4 = reinterpret_cast<const float4 *>(tbuf + d.y);   // S4[2 g + i] = S[4 g + 2 i .. + 1]
                 const float *pl = stage + (size_t)buf * 8 * LP + 4 * tid;
                 mbar_wait(&full_bar[buf], par);
-#pragma unroll 1
-                for (int g4 = 0; g4 < d.x; ++g4) {
+                // chunk g4 = 4 staged positions x 8 images: 3 LDS.128 of tap pairs (broadcast) + 8 LDS.128 of map
+                // values, then 64 FFMA2.  The loads of chunk g4 + 1 are issued before the FMAs of chunk g4.
+                float4 tp[2][3], mv[2][8];
+                auto load_chunk = [&](int g4, float4 (&t)[3], float4 (&m)[8]) {
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) t[i] = S4[2 * g4 + i];
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) m[g] = *reinterpret_cast<const float4 *>(pl + g * LP + 4 * g4);
+                };
+                auto fma_chunk = [&](const float4 (&t)[3], const float4 (&m)[8]) {
                     // pairs (w[x], w[x-1]) of the 6 tap positions this chunk touches
-                    float2 pwr[6];
+                    const float2 pwr[6] = {make_float2(t[0].x, t[0].y), make_float2(t[0].z, t[0].w), make_float2(t[1].x, t[1].y),
+                                           make_float2(t[1].z, t[1].w), make_float2(t[2].x, t[2].y), make_float2(t[2].z, t[2].w)};
 #pragma unroll
-                    for (int i = 0; i < 3; ++i) {
-                        const float4 v = S4[2 * g4 + i];
-                        pwr[2 * i] = make_float2(v.x, v.y); pwr[2 * i + 1] = make_float2(v.z, v.w);
-                    }
+                    for (int g = 0; g < 8; ++g) {
+                        const float mm[4] = {m[g].x, m[g].y, m[g].z, m[g].w};
 #pragma unroll
-                    for (int half = 0; half < 2; ++half) {
-                        float4 mv[4];
-#pragma unroll
-                        for (int q = 0; q < 4; ++q)
-                            mv[q] = *reinterpret_cast<const float4 *>(pl + (half * 4 + q) * LP + 4 * g4);
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const int g = half * 4 + q;
-                            const float mm[4] = {mv[q].x, mv[q].y, mv[q].z, mv[q].w};
-#pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                const float2 m2 = make_float2(mm[i], mm[i]);
-                                acc01[g] = __ffma2_rn(pwr[2 + i], m2, acc01[g]);
-                                acc23[g] = __ffma2_rn(pwr[i], m2, acc23[g]);
-                            }
+                        for (int i = 0; i < 4; ++i) {
+                            const float2 m2 = make_float2(mm[i], mm[i]);
+                            acc01[g] = __ffma2_rn(pwr[2 + i], m2, acc01[g]);
+                            acc23[g] = __ffma2_rn(pwr[i], m2, acc23[g]);
                         }
                     }
+                };
+                const int ng = d.x;
+#if SC_BELT_PREFETCH
+                load_chunk(0, tp[0], mv[0]);
+#pragma unroll 1
+                for (int g4 = 0; g4 < ng; g4 += 2) {
+                    if (g4 + 1 < ng) load_chunk(g4 + 1, tp[1], mv[1]);
+                    fma_chunk(tp[0], mv[0]);
+                    if (g4 + 1 < ng) {
+                        if (g4 + 2 < ng) load_chunk(g4 + 2, tp[0], mv[0]);
+                        fma_chunk(tp[1], mv[1]);
+                    }
                 }
+#else
+#pragma unroll 1
+                for (int g4 = 0; g4 < ng; ++g4) {
+                    load_chunk(g4, tp[0], mv[0]);
+                    fma_chunk(tp[0], mv[0]);
+                }
+#endif
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
                 if (++buf == NBUF) { buf = 0; par ^= 1u; }

@@ -54,10 +54,13 @@ static __device__ __noinline__ unsigned sym_exact_mask(const Dev &P, int r, int 
     return mask;
 }
 
-// Shared-memory slot of staged position i.  A thread owns R adjacent base pixels, so the lanes of a warp
-// read positions R apart: one float4 of padding after every 8 positions makes a stride of 2 or 4
-// positions hit 8 different 16-byte bank groups per quarter warp (stride 1 needs no padding).
-template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) { return R == 1 ? i : i + (i >> 3); }
+// Shared-memory slot (16-byte unit) of staged position i.  A thread owns R adjacent base pixels, so the
+// 8 lanes of a quarter warp (one LDS.128 wavefront) read positions R apart.  XOR-ing the low bits with the
+// index of the 8-position block spreads such a stride over all 8 bank groups for every alignment, with no
+// padding (brute-force checked: 1 wavefront per quarter warp for stride 2 and 4; stride 1 needs nothing).
+template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) {
+    return R == 1 ? i : (R == 2 ? i ^ ((i >> 3) & 1) : i ^ ((i >> 3) & 3));
+}
 
 // Packed fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a; a scalar operand is broadcast by the hardware).
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
@@ -84,9 +87,9 @@ __global__ void __launch_bounds__(NC + kSymProd, 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(R == 1 || R == 2 || R == 4, "R");
     constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);
-    const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 15) & ~(size_t)15));
+    const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 127) & ~(size_t)127));
     __shared__ unsigned long long full_bar[kSymBuf], empty_bar[kSymBuf];
     const int tid = threadIdx.x;
     const int N = P.nside;
@@ -107,7 +110,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     // multiple of 8); the producer warpgroup hands most of its share to the consumer warpgroups
     if (tid >= NC) {
         // ======================================= producers =======================================
-        if (NC == 256) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (NC == 256) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         const int pt = tid - NC;
         const int m = pt & 3;                            // quadrant image staged by this thread
         for (int row = 0; row < nrows; ++row) {
@@ -117,31 +120,46 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
             for (int step = 0; step < nsteps; ++step, ++it) {
                 const int buf = it % kSymBuf;
-                mbar_wait(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);      // every consumer warp released it
-                for (int s = 0; s < nsub; ++s) {
+                // runs to stage for this step, worked out BEFORE waiting for the buffer so that the
+                // table reads (global memory) are off the critical path
+                int kq0[kMaxSub], Ls[kMaxSub], nqs[kMaxSub], sn[kMaxSub], ss[kMaxSub];
+                unsigned d0[kMaxSub];
+#pragma unroll
+                for (int s = 0; s < kMaxSub; ++s) {
+                    Ls[s] = 0;
+                    if (s >= nsub) continue;
                     const int ne = __ldg(&tl->sub[s].ne);
                     if (step >= ne) continue;
                     const int r = __ldg(&tl->sub[s].r), k0 = __ldg(&tl->sub[s].k0), n = __ldg(&tl->sub[s].n);
                     const int soff = __ldg(&tl->sub[s].soff);
-                    const PairEnt pe = F.pairs[__ldg(&tl->sub[s].e0) + step];
+                    const PairEnt *pe = F.pairs + (__ldg(&tl->sub[s].e0) + step);
+                    const int2 pa = __ldg(reinterpret_cast<const int2 *>(&pe->rq));       // rq, hw
+                    const int2 pb = __ldg(reinterpret_cast<const int2 *>(&pe->ipq));      // ipq, shq
+                    const int2 ps = __ldg(reinterpret_cast<const int2 *>(&pe->start_n));  // start_n, start_s
+                    const int hw = pa.y, ipq = pb.x, shq = pb.y;
                     const int ips = r < N ? r : N;
                     const int shs = (r >= N) ? ((r - N) & 1) : 0;
                     const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
-                    const int nq = 4 * pe.ipq;
+                    const int nq = 4 * ipq;
                     const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
-                    const int w0 = div_fast(a0s * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) - pe.hw;
-                    const int L = div_fast(als * pe.ipq + pe.shq * ips, 2 * ips, M0s, rem_unused) + pe.hw + R - w0;
-                    int kq0 = w0 + m * pe.ipq + nq;      // in [0, 2 nq)
-                    if (kq0 >= nq) kq0 -= nq;
-                    const unsigned d0 = stage_sh + (unsigned)((buf * B * 2) * Ltot + soff) * 16u + 4u * m;
-                    for (int i = pt >> 2; i < L; i += kSymProd / 4) {
-                        int kq = kq0 + i;                // L < nq: one wrap at most
-                        if (kq >= nq) kq -= nq;
-                        const unsigned d = d0 + 16u * (unsigned)slot_of_pos<R>(i);
+                    const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw;
+                    Ls[s] = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R - w0;
+                    int k = w0 + m * ipq + nq;           // in [0, 2 nq)
+                    if (k >= nq) k -= nq;
+                    kq0[s] = k; nqs[s] = nq; sn[s] = ps.x; ss[s] = ps.y;
+                    d0[s] = stage_sh + (unsigned)((buf * B * 2) * Ltot + soff) * 16u + 4u * m;
+                }
+                mbar_wait_sleep(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);   // every consumer warp released it
+#pragma unroll
+                for (int s = 0; s < kMaxSub; ++s) {
+                    for (int i = pt >> 2; i < Ls[s]; i += kSymProd / 4) {
+                        int kq = kq0[s] + i;             // L < nq: one wrap at most
+                        if (kq >= nqs[s]) kq -= nqs[s];
+                        const unsigned d = d0[s] + 16u * (unsigned)slot_of_pos<R>(i);
 #pragma unroll
                         for (int b = 0; b < B; ++b) {
-                            cp_async4_s(d + (unsigned)(b * 2 * Ltot) * 16u, io.in[b] + pe.start_n + kq);
-                            cp_async4_s(d + (unsigned)((b * 2 + 1) * Ltot) * 16u, io.in[b] + pe.start_s + kq);
+                            cp_async4_s(d + (unsigned)(b * 2 * Ltot) * 16u, io.in[b] + sn[s] + kq);
+                            cp_async4_s(d + (unsigned)((b * 2 + 1) * Ltot) * 16u, io.in[b] + ss[s] + kq);
                         }
                     }
                 }
@@ -153,7 +171,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     }
 
     // ========================================= consumers =========================================
-    if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+    if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
     const int warp = tid >> 5, lane = tid & 31;
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
     const float tmax = P.tmax, eps = P.eps;
@@ -432,7 +450,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const int ntab_s = P.ntab - 1 + kTabPad;
-    const size_t tab_bytes = ((size_t)ntab_s * 8 + 15) & ~(size_t)15;
+    const size_t tab_bytes = ((size_t)ntab_s * 8 + 127) & ~(size_t)127;
     if (tab_bytes + 8192 > (size_t)smem_optin) return nullptr;       // table does not fit: generic only
 
     auto ipof = [&](int r) { return r < N ? r : (r <= 3 * N ? N : 4 * N - r); };
@@ -581,7 +599,6 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
                     sb.Lcap = std::max(sb.Lcap, L);
                     sb.work += (double)(2 * pe.hw + R);
                 }
-                if (R > 1) sb.Lcap = sb.Lcap + (sb.Lcap >> 3) + 1;      // slot_of_pos padding
                 sb.Lcap = (sb.Lcap + 7) & ~7;
                 sb.work *= sb.nw;
                 return sb;
