@@ -176,7 +176,9 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
     const float tmax = P.tmax, eps = P.eps;
     // shared-memory byte address of tab[0] minus 8 kMagicBits (mod 2^32): tab[bits - kMagicBits] = [tab_sh + 8 bits]
-    const unsigned tab_sh = smem_u32(tab) - kMagicBits * 8u;
+    // (kept opaque: otherwise the compiler re-derives it from the CTA's shared window inside the pair loop)
+    unsigned tab_sh = smem_u32(tab) - kMagicBits * 8u;
+    asm volatile("mov.u32 %0, %0;" : "+r"(tab_sh));
 
     for (int row = 0; row < nrows; ++row) {
         const int tile = snake_tile(row, G, bid);
@@ -229,7 +231,10 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 const int i0 = kc - w0;
                 unsigned pn[B];                          // shared address of this sub-tile's north plane, map b
 #pragma unroll
-                for (int b = 0; b < B; ++b) pn[b] = stage_sh + (unsigned)(((buf * B + b) * 2) * Ltot + me.soff) * 16u;
+                for (int b = 0; b < B; ++b) {
+                    pn[b] = stage_sh + (unsigned)(((buf * B + b) * 2) * Ltot + me.soff) * 16u;
+                    asm volatile("mov.u32 %0, %0;" : "+r"(pn[b]));      // one register, not re-derived per position
+                }
                 const unsigned south = (unsigned)Ltot * 16u;
                 float2 acc[R][B][4];
 #pragma unroll
