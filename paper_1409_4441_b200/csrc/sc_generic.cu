@@ -122,6 +122,90 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
     }
 }
 
+// Same arithmetic with one WARP per output pixel: 4 groups of 8 lanes take every 4th input ring, the 8
+// lanes of a group share its azimuthal window, and the partial sums are combined with warp shuffles.  Used for the few thousand pixels next to
+// the poles, where one thread per pixel leaves the GPU almost empty (latency bound).
+template <int B>
+__global__ void __launch_bounds__(128)
+generic_warp_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1) {
+    const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int na = a1 - a0;
+    int p;
+    if (wid < na) p = a0 + wid;
+    else if (wid - na < b1 - b0) p = b0 + (wid - na);
+    else return;                                             // whole warp
+    const int grp = lane >> 3, gl = lane & 7;
+
+    float tot[B];
+#pragma unroll
+    for (int b = 0; b < B; ++b) tot[b] = 0.f;
+    int kp;
+    const int rp = ring_of_pixel(P, p, kp);
+    const double zp = P.z[rp - 1], sp = P.s[rp - 1];
+    const double phip = P.phi0[rp - 1] + (double)kp * P.dphi[rp - 1];
+    const int r_lo = P.rlo[rp - 1], r_hi = P.rhi[rp - 1];
+
+    for (int rq = r_lo + grp; rq <= r_hi; rq += 4) {
+        const double zq = P.z[rq - 1], sq = P.s[rq - 1];
+        double A64 = 1.0 - (zp * zq + sp * sq);
+        if (A64 < 0.0) A64 = 0.0;
+        const float Af = (float)(A64 * P.scale);
+        const float Bf = (float)(sp * sq * P.scale);
+        const float wmax = (P.tmax + P.eps - Af) / Bf;
+        if (!(wmax >= 0.f)) continue;                        // whole ring beyond theta_max
+        const int nq = P.npr[rq - 1];
+        const int startq = P.start[rq - 1];
+        const double dphiq = P.dphi[rq - 1];
+        const float dphiq_f = (float)dphiq;
+        const double xq = (phip - P.phi0[rq - 1]) / dphiq;
+        int kc = (int)rint(xq);
+        const float dc = (float)((P.phi0[rq - 1] + (double)kc * dphiq) - phip);
+        kc %= nq; if (kc < 0) kc += nq;
+        int jlo, jcnt;
+        if (wmax >= 2.f) { jlo = -(nq / 2); jcnt = nq; }
+        else {
+            const float H = 2.f * asinf(sqrtf(0.5f * wmax));
+            const int hw = (int)(H / dphiq_f * 1.0001f + 1.5f) + 1;
+            if (2 * hw + 1 >= nq) { jlo = -(nq / 2); jcnt = nq; }
+            else { jlo = -hw; jcnt = 2 * hw + 1; }
+        }
+        float racc[B];
+#pragma unroll
+        for (int b = 0; b < B; ++b) racc[b] = 0.f;
+        for (int jj = gl; jj < jcnt; jj += 8) {
+            const int j = jlo + jj;
+            int kq = kc + j;
+            if (kq < 0) kq += nq; else if (kq >= nq) kq -= nq;
+            const float d = fmaf((float)j, dphiq_f, dc);
+            const float sh = sinf(0.5f * d);
+            const float w = 2.f * sh * sh;
+            const float t = fmaf(Bf, w, Af);
+            bool in = t < P.tmax - P.eps;
+            float tt = t;
+            if (!in && t <= P.tmax + P.eps) {
+                in = exact_included(P, rp, kp, rq, kq, t, nullptr);
+                tt = fminf(t, P.tmax);
+            }
+            if (in) {
+                int i = (int)tt;
+                if (i > P.ntab - 2) i = P.ntab - 2;
+                const float2 e = __ldg(&P.tab[i]);
+                const float K = fmaf(tt, e.y, e.x);
+#pragma unroll
+                for (int b = 0; b < B; ++b) racc[b] = fmaf(K, __ldg(&io.in[b][startq + kq]), racc[b]);
+            }
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) tot[b] += racc[b];
+    }
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        float v = tot[b];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) io.out[b][p] = v * P.omega;
+    }
+}
+
 // host launchers -----------------------------------------------------------------------------
 cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1,
                                 cudaStream_t st) {
@@ -134,6 +218,21 @@ cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int
         case 2: generic_kernel<2, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
         case 3: generic_kernel<3, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
         case 4: generic_kernel<4, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_generic_conv_warp(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1,
+                                     cudaStream_t st) {
+    const int n = (a1 - a0) + (b1 - b0);
+    if (n <= 0) return cudaSuccess;
+    const int threads = 128, blocks = (n + 3) / 4;
+    switch (B) {
+        case 1: generic_warp_kernel<1><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 2: generic_warp_kernel<2><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 3: generic_warp_kernel<3><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 4: generic_warp_kernel<4><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -14,6 +14,7 @@
 
 namespace sc {
 cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1, cudaStream_t st);
+cudaError_t launch_generic_conv_warp(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1, cudaStream_t st);
 cudaError_t launch_generic_count(const Dev &P, int *count_dev, unsigned long long *sig_dev, const Audit *au, cudaStream_t st);
 struct FastPlan;
 FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std::vector<double> &s,
@@ -350,7 +351,7 @@ sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *c
             const int pr = plan->polar_rings;
             if (pr > 0) {
                 const int np = 2 * pr * (pr + 1);          // pixels in rings 1..pr
-                SC_CUDA(sc::launch_generic_conv(D, io, nb, 0, np, D.npix - np, D.npix, st));
+                SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, st));
                 ++launches;
             }
             int nl = 0;
