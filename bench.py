@@ -48,12 +48,51 @@ def _workload_name(cfg):
             f"B={cfg.batch} fp32 N(0,1) map(s), {cfg.kernel} kernel, {cfg.n_table}-sample cos(theta) table")
 
 
+def _traffic(cfg_name, kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu --set full capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    try:
+        with open(path) as f:
+            for line in f:
+                a = [x.strip() for x in line.split(",")]
+                if len(a) >= 3 and a[0] == cfg_name and a[1] == kernel:
+                    return float(a[2])
+    except Exception:
+        pass
+    return None
+
+
 def _sm_max_mhz():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             return float(json.load(f)["sm_max_mhz"]), "MEASURED_PEAKS.json sm_max_mhz"
     except Exception:
         return 1965.0, "fallback 1965 MHz (B200_PROFILING.md)"
+
+
+def _ring_start(N, i):
+    """First RING pixel of ring i (1-based); i = 4N gives N_pix.  Index arithmetic only."""
+    if i < N:
+        return 2 * i * (i - 1)
+    if i <= 3 * N:
+        return 2 * N * (N - 1) + (i - N) * 4 * N
+    m = 4 * N - i
+    return 12 * N * N - 2 * m * (m + 1)
+
+
+def _pairs_per_kernel(plan, N):
+    """Included pairs of the pixels each kernel writes (from the plan's per-pixel neighbour counts)."""
+    import torch
+    cnt, _ = plan.neighbour_counts(want_sig=False)
+    cs = torch.zeros(cnt.numel() + 1, dtype=torch.int64, device=cnt.device)
+    cs[1:] = torch.cumsum(cnt.to(torch.int64), 0)
+    part = plan.partition()
+    pr, fb = part["polar_rings"], part["first_belt_ring"]
+    rng = lambda a, b: int(cs[_ring_start(N, b)] - cs[_ring_start(N, a)]) if b > a else 0   # rings a .. b-1
+    polar = rng(1, pr + 1) + rng(4 * N - pr, 4 * N)
+    belt = rng(fb, 4 * N - fb + 1) if fb <= 2 * N else 0
+    total = int(cs[-1])
+    return {"generic_warp_kernel": polar, "sym_kernel": total - polar - belt, "belt_kernel": belt}, part
 
 
 class ClockSampler(threading.Thread):
@@ -144,10 +183,11 @@ def run_ours(args, cfg, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     import paper_1409_4441_b200 as sc
+    from paper_1409_4441_b200 import dist as scdist
 
     T = gen.table_for(cfg)
     # every rank gets its own maps (seed offset): independent problems, weak scaling
-    seeds = [s + 1000 * rank for s in cfg.seeds]
+    seeds = scdist.rank_seeds(cfg.seeds, rank)
     host_maps = [gen.noise_map(cfg.npix, s) for s in seeds]
     if cfg.ylm_map:
         host_maps.append(gen.ylm_map(cfg.nside, seed=1000 + cfg.seeds[0]).astype(np.float32))
@@ -191,6 +231,16 @@ def run_ours(args, cfg, rank, world, local_rank):
     step_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
     total_ms = ev[0].elapsed_time(ev[-1])
 
+    # per-kernel device times (events on the launching stream around every kernel; separate pass)
+    kern_ms = {}
+    nprof = max(3, min(args.steps, 10))
+    if args.path == "auto":
+        for _ in range(nprof):
+            for k, v in plan.convolve_profile(dev_in, dev_out).items():
+                kern_ms[k] = kern_ms.get(k, 0.0) + v / nprof
+        kern_pairs, part = _pairs_per_kernel(plan, cfg.nside)
+    barrier()
+
     # end to end through the HOST-buffer entry point (pinned host memory, copies inside the timing)
     pin_in = [torch.from_numpy(m).pin_memory() for m in host_maps]
     pin_out = [torch.empty(cfg.npix, dtype=torch.float32).pin_memory() for _ in range(B)]
@@ -207,11 +257,8 @@ def run_ours(args, cfg, rank, world, local_rank):
     if not np.isfinite(checksum) or checksum == 0.0:
         raise SystemExit("non-finite or zero output")
 
-    t = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_s = float(t[0]), float(t[1])
-    pairs_step_all = total_pairs * B * world
+    # max over ranks of the times, sum over ranks of the work
+    (total_ms, e2e_s), pairs_step_all = scdist.combine_timing([total_ms, e2e_s], total_pairs * B)
     value = pairs_step_all * args.steps / (total_ms * 1e-3)
     e2e_value = pairs_step_all * e2e_steps / e2e_s
 
@@ -221,15 +268,14 @@ def run_ours(args, cfg, rank, world, local_rank):
         # algorithmic FMAs: 6 per pair at B = 1 (3 geometry + table coordinate + lerp + accumulate),
         # 5 + B per pair geometry with a batch
         fma_per_step = total_pairs * (5 + B)
-        kern_ms = float(np.mean(step_ms))
-        achieved = fma_per_step / (kern_ms * 1e-3)
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tp):
-            try:
-                traffic = json.load(open(tp)).get(cfg.name)
-            except Exception:
-                traffic = None
+        step_mean_ms = float(np.mean(step_ms))
+        if kern_ms:
+            dom = max(kern_ms, key=kern_ms.get)                       # the dominant kernel of the step
+            dom_ms, dom_pairs = kern_ms[dom], kern_pairs[dom]
+        else:
+            dom, dom_ms, dom_pairs = "generic_kernel", step_mean_ms, total_pairs
+        achieved = dom_pairs * (5 + B) / (dom_ms * 1e-3)
+        traffic = _traffic(cfg.name, dom)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -243,11 +289,16 @@ def run_ours(args, cfg, rank, world, local_rank):
                         "d2h_bytes_per_step": 4 * cfg.npix * B, "ms_per_step": 1e3 * e2e_s / e2e_steps,
                         "launches_per_step": e2e_launches},
                 "gpu_launches": launches,
-                "roofline": {"bound": "alu", "achieved": achieved / 1e9, "peak": peak_fma / 1e9,
+                "roofline": {"bound": "alu", "kernel": dom, "achieved": achieved / 1e9, "peak": peak_fma / 1e9,
                              "unit": "GFMA/s", "frac": achieved / peak_fma, "traffic": traffic,
+                             "kernel_ms": dom_ms, "kernel_pairs": dom_pairs,
                              "peak_source": f"{N_SM} SMs x {LANES} FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
-                             "model": f"{5 + B} algorithmic FMA per pair geometry (5 + B), whole step / all launches",
-                             "min_step_ms": float(np.min(step_ms))}}
+                             "model": f"{5 + B} algorithmic FMA per pair geometry (5 + B) x the pairs of the "
+                                      f"pixels this kernel writes / its mean launch time (CUDA events)",
+                             "kernels_ms": kern_ms, "kernels_pairs": kern_pairs if kern_ms else None,
+                             "step": {"achieved": fma_per_step / (step_mean_ms * 1e-3) / 1e9,
+                                      "frac": fma_per_step / (step_mean_ms * 1e-3) / peak_fma,
+                                      "ms": step_mean_ms, "min_ms": float(np.min(step_ms))}}}
         if not args.no_cpu and world == 1:
             v, oi = oracle_sample(cfg, args.cpu_seconds)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": oi["cores"], "kind": "oracle",

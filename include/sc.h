@@ -129,6 +129,30 @@ sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uin
 sc_status sc_debug_stats(const sc_plan *plan, int64_t *n_uncertain, double *max_t_err,
                          double *guard_band);
 
+/*
+ * sc_convolve_profile -- measurement only: the same launches as sc_convolve with CUDA events recorded
+ * on `cuda_stream` around every kernel; synchronises the stream and returns the device time of each
+ * kernel of the step, summed over batch chunks:
+ *   ms[SC_K_POLAR]  generic_warp_kernel  (rings next to the poles)
+ *   ms[SC_K_SYM]    sym_kernel           (polar caps and the cap/belt transition)
+ *   ms[SC_K_BELT]   belt_kernel          (equatorial belt stencil)
+ * ms: HOST array of SC_K_COUNT floats (milliseconds; 0 for a kernel this plan does not launch).
+ */
+enum { SC_K_POLAR = 0, SC_K_SYM = 1, SC_K_BELT = 2, SC_K_COUNT = 3 };
+sc_status sc_convolve_profile(const sc_plan *plan, const float *const *in_maps,
+                              float *const *out_maps, int B, void *cuda_stream, float *ms);
+
+/*
+ * sc_plan_partition -- which pixels each kernel of the AUTO path writes (HOST outputs, may be NULL).
+ * With N = nside, base rings are 1 .. 2N and every base ring r stands for itself and its southern
+ * mirror 4N - r:
+ *   polar_rings      base rings 1 .. polar_rings                     -> generic_warp_kernel
+ *   first_belt_ring  base rings polar_rings + 1 .. first_belt_ring-1 -> sym_kernel,
+ *                    base rings first_belt_ring .. 2N                 -> belt_kernel
+ *                    (2N + 1 if the plan has no belt kernel; polar_rings = 2N if it has no fast path)
+ */
+sc_status sc_plan_partition(const sc_plan *plan, int *polar_rings, int *first_belt_ring);
+
 /* Kernel launches enqueued by the last sc_convolve / sc_convolve_host on this plan. */
 int sc_last_launch_count(const sc_plan *plan);
 

@@ -10,7 +10,11 @@ SC_ORDER_RING, SC_ORDER_NESTED = 0, 1
 SC_PATH_AUTO, SC_PATH_GENERIC = 0, 1
 
 # every symbol include/sc.h declares
-EXPORTS = ("sc_plan_create", "sc_convolve", "sc_convolve_host", "sc_plan_destroy", "sc_plan_set_path",
+SC_K_POLAR, SC_K_SYM, SC_K_BELT, SC_K_COUNT = 0, 1, 2, 3
+KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
+
+EXPORTS = ("sc_plan_create", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
+           "sc_plan_destroy", "sc_plan_set_path",
            "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_last_launch_count",
            "sc_status_string", "sc_last_cuda_error", "sc_version")
 
@@ -38,6 +42,8 @@ def lib():
         l.sc_plan_create.argtypes = [C.POINTER(vp), i32, i32, vp, i32, dbl, i32]
         l.sc_convolve.argtypes = [vp, vp, vp, i32, vp]
         l.sc_convolve_host.argtypes = [vp, vp, vp, i32]
+        l.sc_convolve_profile.argtypes = [vp, vp, vp, i32, vp, vp]
+        l.sc_plan_partition.argtypes = [vp, vp, vp]
         l.sc_plan_destroy.argtypes = [vp]
         l.sc_plan_set_path.argtypes = [vp, i32]
         l.sc_plan_info.argtypes = [vp, vp, vp, vp, vp]
@@ -87,6 +93,22 @@ def sc_convolve_host(plan, in_ptrs, out_ptrs):
         raise ValueError("in/out batch mismatch")
     _chk(lib().sc_convolve_host(plan, _ptr_array(in_ptrs), _ptr_array(out_ptrs), len(in_ptrs)),
          "sc_convolve_host")
+
+
+def sc_convolve_profile(plan, in_ptrs, out_ptrs, stream=0):
+    """Measurement only: one step with events around every kernel -> per-kernel ms (tuple of SC_K_COUNT)."""
+    if len(in_ptrs) != len(out_ptrs):
+        raise ValueError("in/out batch mismatch")
+    ms = (C.c_float * SC_K_COUNT)()
+    _chk(lib().sc_convolve_profile(plan, _ptr_array(in_ptrs), _ptr_array(out_ptrs), len(in_ptrs),
+                                   C.c_void_p(int(stream) or None), ms), "sc_convolve_profile")
+    return tuple(float(x) for x in ms)
+
+
+def sc_plan_partition(plan):
+    pr, fb = C.c_int(0), C.c_int(0)
+    _chk(lib().sc_plan_partition(plan, C.byref(pr), C.byref(fb)), "sc_plan_partition")
+    return dict(polar_rings=pr.value, first_belt_ring=fb.value)
 
 
 def sc_plan_destroy(plan):
@@ -160,6 +182,16 @@ class Plan:
         sc_convolve(self.handle, [m.data_ptr() for m in maps], [o.data_ptr() for o in out],
                     torch.cuda.current_stream().cuda_stream)
         return out
+
+    def convolve_profile(self, maps, out):
+        """Measurement only: one step, returns {kernel name: device ms} (synchronises the stream)."""
+        import torch
+        ms = sc_convolve_profile(self.handle, [m.data_ptr() for m in maps], [o.data_ptr() for o in out],
+                                 torch.cuda.current_stream().cuda_stream)
+        return dict(zip(KERNEL_NAMES, ms))
+
+    def partition(self):
+        return sc_plan_partition(self.handle)
 
     def convolve_host(self, maps, out=None):
         """maps: list of host fp32 numpy arrays or CPU tensors (N_pix) -> list of numpy arrays."""

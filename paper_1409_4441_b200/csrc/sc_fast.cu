@@ -382,6 +382,7 @@ struct FastPlan {
     int *counter = nullptr;
     int ntab_s = 0;
     int polar = 0;
+    int first_belt = 0;           // base rings first_belt .. 2N go to the belt kernel (2N + 1: none)
     FastCfg cfg[kMaxB + 1];
     int nsm = 148;
     // belt kernel
@@ -405,7 +406,8 @@ static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P
     return cudaGetLastError();
 }
 
-cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches) {
+cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches,
+                          cudaEvent_t *ev) {
     *launches = 0;
     if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return cudaErrorInvalidValue;
     const FastCfg &c = fp->cfg[B];
@@ -422,12 +424,16 @@ cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cud
 #undef SC_SYM_CASE
     if (e != cudaSuccess) return e;
     *launches = c.ntiles > 0 ? 1 : 0;
+    if (ev && (e = cudaEventRecord(ev[0], st)) != cudaSuccess) return e;      // end of the sym kernel
     if (fp->belt_ok) {
         e = launch_belt(P, fp->belt, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
         if (e == cudaSuccess) ++*launches;
     }
+    if (ev && e == cudaSuccess) e = cudaEventRecord(ev[1], st);              // end of the belt kernel
     return e;
 }
+
+int fast_first_belt_ring(const FastPlan *fp) { return fp->first_belt; }
 
 bool fast_available(const FastPlan *fp, int B) { return fp && B >= 1 && B <= kMaxB && fp->cfg[B].ok; }
 
@@ -660,6 +666,8 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             break;
         }
     }
+    fp->first_belt = 2 * N + 1;
+    for (int r = 2 * N; r > polar && is_belt[r]; --r) fp->first_belt = r;
     *polar_rings = polar;
     return fp;
 }

@@ -20,7 +20,8 @@ struct FastPlan;
 FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std::vector<double> &s,
                            int max_batch, int *polar_rings, cudaError_t *err);
 void fast_plan_destroy(FastPlan *fp);
-cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches);
+cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches, cudaEvent_t *ev);
+int fast_first_belt_ring(const FastPlan *fp);
 bool fast_available(const FastPlan *fp, int B);
 }  // namespace sc
 
@@ -328,8 +329,9 @@ sc_status sc_debug_stats(const sc_plan *plan, int64_t *n_uncertain, double *max_
 
 int sc_last_launch_count(const sc_plan *plan) { return plan ? plan->last_launches : 0; }
 
-sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *const *out_maps, int B,
-                      void *cuda_stream) {
+// ev (optional): 4 events recorded before the polar kernel and after each of the three kernels
+static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps, float *const *out_maps, int B,
+                               void *cuda_stream, cudaEvent_t *ev, float *ms) {
     if (!plan || !in_maps || !out_maps || B < 1) return SC_ERR_INVALID_ARG;
     for (int b = 0; b < B; ++b) {
         if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
@@ -343,9 +345,11 @@ sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *c
         const int nb = std::min(sc::kMaxB, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
+        if (ev) SC_CUDA(cudaEventRecord(ev[0], st));
         if (plan->path == SC_PATH_GENERIC || !sc::fast_available(plan->fast, nb)) {
             SC_CUDA(sc::launch_generic_conv(D, io, nb, 0, D.npix, 0, 0, st));
             ++launches;
+            if (ev) { SC_CUDA(cudaEventRecord(ev[1], st)); SC_CUDA(cudaEventRecord(ev[2], st)); SC_CUDA(cudaEventRecord(ev[3], st)); }
         } else {
             // rings next to the poles: generic kernel; everything else: fast kernels
             const int pr = plan->polar_rings;
@@ -354,12 +358,47 @@ sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *c
                 SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, st));
                 ++launches;
             }
+            if (ev) SC_CUDA(cudaEventRecord(ev[1], st));
             int nl = 0;
-            SC_CUDA(sc::fast_convolve(plan->fast, D, io, nb, st, &nl));
+            SC_CUDA(sc::fast_convolve(plan->fast, D, io, nb, st, &nl, ev ? ev + 2 : nullptr));
             launches += nl;
+        }
+        if (ev) {
+            SC_CUDA(cudaEventSynchronize(ev[3]));
+            for (int k = 0; k < SC_K_COUNT; ++k) {
+                float t = 0.f;
+                SC_CUDA(cudaEventElapsedTime(&t, ev[k], ev[k + 1]));
+                ms[k] += t;
+            }
         }
     }
     plan->last_launches = launches;
+    return SC_OK;
+}
+
+sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *const *out_maps, int B,
+                      void *cuda_stream) {
+    return convolve_impl(plan, in_maps, out_maps, B, cuda_stream, nullptr, nullptr);
+}
+
+sc_status sc_convolve_profile(const sc_plan *plan, const float *const *in_maps, float *const *out_maps, int B,
+                              void *cuda_stream, float *ms) {
+    if (!ms) return SC_ERR_INVALID_ARG;
+    cudaEvent_t ev[SC_K_COUNT + 1] = {};
+    for (int k = 0; k < SC_K_COUNT; ++k) ms[k] = 0.f;
+    sc_status st = SC_OK;
+    for (int k = 0; k <= SC_K_COUNT; ++k)
+        if (!cuda_ok(cudaEventCreate(&ev[k]), "cudaEventCreate")) st = SC_ERR_CUDA;
+    if (st == SC_OK) st = convolve_impl(plan, in_maps, out_maps, B, cuda_stream, ev, ms);
+    for (int k = 0; k <= SC_K_COUNT; ++k) if (ev[k]) cudaEventDestroy(ev[k]);
+    return st;
+}
+
+sc_status sc_plan_partition(const sc_plan *plan, int *polar_rings, int *first_belt_ring) {
+    if (!plan) return SC_ERR_INVALID_ARG;
+    const int N2 = 2 * plan->dev.nside;
+    if (polar_rings) *polar_rings = plan->fast ? plan->polar_rings : N2;
+    if (first_belt_ring) *first_belt_ring = plan->fast ? sc::fast_first_belt_ring(plan->fast) : N2 + 1;
     return SC_OK;
 }
 

@@ -254,6 +254,30 @@ def test_batch_chunking_and_host_entry(sc):
         _check_values(batch[b], ref[b], f"batch6 map{b}")
 
 
+def test_profile_entry_and_partition(sc):
+    """sc_convolve_profile runs the same launches as sc_convolve (bit-identical output) and reports a
+    positive device time for every kernel the plan uses; sc_plan_partition is consistent with them."""
+    import torch
+    cfg = gen.config(3)
+    T = gen.table_for(cfg)
+    m = torch.from_numpy(gen.noise_map(cfg.npix, 77)).cuda()
+    with sc.Plan(cfg.nside, T, cfg.theta_max, 1) as plan:
+        a = plan.convolve([m])[0]
+        b = torch.empty_like(m)
+        ms = plan.convolve_profile([m], [b])
+        part = plan.partition()
+        torch.cuda.synchronize()
+        assert torch.equal(a, b)
+        N = cfg.nside
+        assert 0 < part["polar_rings"] < N and part["polar_rings"] < part["first_belt_ring"] <= 2 * N
+        assert set(ms) == set(sc.KERNEL_NAMES)
+        assert all(v > 0 for v in ms.values()), ms
+        assert sc.sc_last_launch_count(plan.handle) == 3
+        plan.set_path(sc.SC_PATH_GENERIC)
+        ms = plan.convolve_profile([m], [b])
+        assert ms["generic_warp_kernel"] > 0.1 and ms["belt_kernel"] < 0.01 and ms["sym_kernel"] < 0.01
+
+
 def test_knife_edge_host_adjudication(sc, monkeypatch):
     """Widen the knife-edge band so that many pairs are decided on the host with the host libm;
     sets must still equal the oracle's and the override list must be in use."""
