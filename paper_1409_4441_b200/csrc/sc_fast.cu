@@ -406,29 +406,42 @@ static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P
     return cudaGetLastError();
 }
 
-cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches,
-                          cudaEvent_t *ev) {
+// which: bit 0 = sym kernel, bit 1 = belt kernel (the two write disjoint pixels and may run on different streams)
+cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches) {
     *launches = 0;
     if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return cudaErrorInvalidValue;
     const FastCfg &c = fp->cfg[B];
-    cudaError_t e = cudaErrorInvalidValue;
-    // more than 256 consumer threads per CTA leave 112 registers per thread, up to 256 threads 200
+    cudaError_t e = cudaSuccess;
+    if (which & 1) {
+        e = cudaErrorInvalidValue;
 #define SC_SYM_CASE(BB, RR)                                                                  \
     if (B == BB && c.R == RR)                                                                \
         e = c.threads == 256 ? launch_sym<BB, RR, 256>(fp, c, P, io, st)                     \
                              : launch_sym<BB, RR, 128>(fp, c, P, io, st);
-    SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
-    SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
-    SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
-    SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
+        SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
+        SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
+        SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
+        SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
 #undef SC_SYM_CASE
-    if (e != cudaSuccess) return e;
-    *launches = c.ntiles > 0 ? 1 : 0;
-    if (ev && (e = cudaEventRecord(ev[0], st)) != cudaSuccess) return e;      // end of the sym kernel
-    if (fp->belt_ok) {
+        if (e != cudaSuccess) return e;
+        *launches += c.ntiles > 0 ? 1 : 0;
+    }
+    if ((which & 2) && fp->belt_ok) {
         e = launch_belt(P, fp->belt, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
         if (e == cudaSuccess) ++*launches;
     }
+    return e;
+}
+
+cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches,
+                          cudaEvent_t *ev) {
+    int n1 = 0, n2 = 0;
+    cudaError_t e = fast_launch(fp, P, io, B, 1, st, &n1);
+    *launches = n1;
+    if (e != cudaSuccess) return e;
+    if (ev && (e = cudaEventRecord(ev[0], st)) != cudaSuccess) return e;      // end of the sym kernel
+    e = fast_launch(fp, P, io, B, 2, st, &n2);
+    *launches += n2;
     if (ev && e == cudaSuccess) e = cudaEventRecord(ev[1], st);              // end of the belt kernel
     return e;
 }

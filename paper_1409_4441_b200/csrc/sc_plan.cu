@@ -22,6 +22,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
 void fast_plan_destroy(FastPlan *fp);
 cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches, cudaEvent_t *ev);
 int fast_first_belt_ring(const FastPlan *fp);
+cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches);
 bool fast_available(const FastPlan *fp, int B);
 }  // namespace sc
 
@@ -87,7 +88,8 @@ struct sc_plan {
     // end-to-end staging
     float *stage_in = nullptr, *stage_out = nullptr;
     int stage_maps = 0;
-    cudaStream_t own_stream = nullptr;
+    cudaStream_t own_stream = nullptr, comp_stream = nullptr, d2h_stream = nullptr;
+    cudaEvent_t ev_belt_in = nullptr, ev_all_in = nullptr, ev_belt_done = nullptr, ev_rest_done = nullptr, ev_prev = nullptr;
     mutable int last_launches = 0;
     sc::FastPlan *fast = nullptr;
     int polar_rings = 0;                       // rings 1..polar_rings and their southern mirrors use the generic kernel
@@ -299,6 +301,10 @@ sc_status sc_plan_destroy(sc_plan *plan) {
     if (plan->stage_in) cudaFree(plan->stage_in);
     if (plan->stage_out) cudaFree(plan->stage_out);
     if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
+    if (plan->comp_stream) cudaStreamDestroy(plan->comp_stream);
+    if (plan->d2h_stream) cudaStreamDestroy(plan->d2h_stream);
+    for (cudaEvent_t e : {plan->ev_belt_in, plan->ev_all_in, plan->ev_belt_done, plan->ev_rest_done, plan->ev_prev})
+        if (e) cudaEventDestroy(e);
     delete plan;
     return SC_OK;
 }
@@ -416,16 +422,76 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
         plan->stage_maps = nm;
     }
     if (!plan->own_stream) SC_CUDA(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
-    std::vector<const float *> in(B); std::vector<float *> out(B);
-    for (int b = 0; b < B; ++b) {
-        in[b] = plan->stage_in + npix * b; out[b] = plan->stage_out + npix * b;
-        SC_CUDA(cudaMemcpyAsync(plan->stage_in + npix * b, in_maps_host[b], npix * 4, cudaMemcpyHostToDevice, plan->own_stream));
+    const sc::Dev &D = plan->dev;
+    const int N = D.nside;
+    const int fb = plan->fast ? sc::fast_first_belt_ring(plan->fast) : 2 * N + 1;
+    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && fb <= 2 * N;
+    if (!pipelined) {
+        std::vector<const float *> in(B); std::vector<float *> out(B);
+        for (int b = 0; b < B; ++b) {
+            in[b] = plan->stage_in + npix * b; out[b] = plan->stage_out + npix * b;
+            SC_CUDA(cudaMemcpyAsync(plan->stage_in + npix * b, in_maps_host[b], npix * 4, cudaMemcpyHostToDevice, plan->own_stream));
+        }
+        sc_status st = sc_convolve(plan, in.data(), out.data(), B, plan->own_stream);
+        if (st != SC_OK) return st;
+        for (int b = 0; b < B; ++b)
+            SC_CUDA(cudaMemcpyAsync(out_maps_host[b], out[b], npix * 4, cudaMemcpyDeviceToHost, plan->own_stream));
+        SC_CUDA(cudaStreamSynchronize(plan->own_stream));
+        return SC_OK;
     }
-    sc_status st = sc_convolve(plan, in.data(), out.data(), B, plan->own_stream);
-    if (st != SC_OK) return st;
-    for (int b = 0; b < B; ++b)
-        SC_CUDA(cudaMemcpyAsync(out_maps_host[b], out[b], npix * 4, cudaMemcpyDeviceToHost, plan->own_stream));
-    SC_CUDA(cudaStreamSynchronize(plan->own_stream));
+
+    // Pipelined: the belt kernel reads only belt rings (N .. 3N) and writes base rings fb .. 2N and
+    // their mirrors, so it can start as soon as the belt rows have arrived and its output can travel
+    // back while the cap kernels still run.  Three streams (copy in, compute, copy out) and events.
+    if (!plan->comp_stream) {
+        SC_CUDA(cudaStreamCreateWithFlags(&plan->comp_stream, cudaStreamNonBlocking));
+        SC_CUDA(cudaStreamCreateWithFlags(&plan->d2h_stream, cudaStreamNonBlocking));
+        for (cudaEvent_t *e : {&plan->ev_belt_in, &plan->ev_all_in, &plan->ev_belt_done, &plan->ev_rest_done, &plan->ev_prev})
+            SC_CUDA(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    }
+    cudaStream_t s_in = plan->own_stream, s_c = plan->comp_stream, s_out = plan->d2h_stream;
+    const size_t belt_lo = (size_t)D.ncap, belt_hi = npix - (size_t)D.ncap;                 // input rows of the belt kernel
+    const size_t ob_lo = (size_t)plan->rings[fb - 1].start;                                // its output rows
+    const size_t ob_hi = (4 * N - fb + 1 <= 4 * N - 1) ? (size_t)plan->rings[4 * N - fb].start : npix;
+    const int pr = plan->polar_rings;
+    int launches = 0;
+    for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
+        const int nb = std::min(sc::kMaxB, B - b0);
+        sc::Maps io{};
+        for (int b = 0; b < nb; ++b) { io.in[b] = plan->stage_in + npix * (b0 + b); io.out[b] = plan->stage_out + npix * (b0 + b); }
+        for (int b = 0; b < nb; ++b)
+            SC_CUDA(cudaMemcpyAsync((float *)io.in[b] + belt_lo, in_maps_host[b0 + b] + belt_lo, (belt_hi - belt_lo) * 4, cudaMemcpyHostToDevice, s_in));
+        SC_CUDA(cudaEventRecord(plan->ev_belt_in, s_in));
+        for (int b = 0; b < nb; ++b) {
+            SC_CUDA(cudaMemcpyAsync((float *)io.in[b], in_maps_host[b0 + b], belt_lo * 4, cudaMemcpyHostToDevice, s_in));
+            SC_CUDA(cudaMemcpyAsync((float *)io.in[b] + belt_hi, in_maps_host[b0 + b] + belt_hi, (npix - belt_hi) * 4, cudaMemcpyHostToDevice, s_in));
+        }
+        SC_CUDA(cudaEventRecord(plan->ev_all_in, s_in));
+
+        int nl = 0;
+        SC_CUDA(cudaStreamWaitEvent(s_c, plan->ev_belt_in, 0));
+        SC_CUDA(sc::fast_launch(plan->fast, D, io, nb, 2, s_c, &nl)); launches += nl;
+        SC_CUDA(cudaEventRecord(plan->ev_belt_done, s_c));
+        SC_CUDA(cudaStreamWaitEvent(s_c, plan->ev_all_in, 0));
+        if (pr > 0) {
+            const int np = 2 * pr * (pr + 1);
+            SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, s_c));
+            ++launches;
+        }
+        SC_CUDA(sc::fast_launch(plan->fast, D, io, nb, 1, s_c, &nl)); launches += nl;
+        SC_CUDA(cudaEventRecord(plan->ev_rest_done, s_c));
+
+        SC_CUDA(cudaStreamWaitEvent(s_out, plan->ev_belt_done, 0));
+        for (int b = 0; b < nb; ++b)
+            SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b] + ob_lo, io.out[b] + ob_lo, (ob_hi - ob_lo) * 4, cudaMemcpyDeviceToHost, s_out));
+        SC_CUDA(cudaStreamWaitEvent(s_out, plan->ev_rest_done, 0));
+        for (int b = 0; b < nb; ++b) {
+            SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b], io.out[b], ob_lo * 4, cudaMemcpyDeviceToHost, s_out));
+            SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b] + ob_hi, io.out[b] + ob_hi, (npix - ob_hi) * 4, cudaMemcpyDeviceToHost, s_out));
+        }
+    }
+    plan->last_launches = launches;
+    SC_CUDA(cudaStreamSynchronize(s_out));
     return SC_OK;
 }
 
