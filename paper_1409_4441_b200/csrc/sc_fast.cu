@@ -82,7 +82,9 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 // Warp-specialised: the first blockDim.x - kSymProd threads are consumers (pair loop), the last
 // kSymProd threads are producers (staging).  They meet only through the full/empty mbarriers of the
 // kSymBuf stage buffers; there is no block-wide barrier after the prologue.
-template <int B, int R, int NC>
+// TOT: per-step partial sums are added to a second accumulator set (pairwise-like summation; needed for
+// discs of thousands of pixels, costs 8 R B registers).
+template <int B, int R, int NC, bool TOT>
 __global__ void __launch_bounds__(NC + kSymProd, 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(R == 1 || R == 2 || R == 4, "R");
@@ -110,7 +112,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     // multiple of 8); the producer warpgroup hands most of its share to the consumer warpgroups
     if (tid >= NC) {
         // ======================================= producers =======================================
-        if (NC == 256) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        if (NC == 256 || NC == 384) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         const int pt = tid - NC;
         const int m = pt & 3;                            // quadrant image staged by this thread
         for (int row = 0; row < nrows; ++row) {
@@ -172,6 +174,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 
     // ========================================= consumers =========================================
     if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    if (NC == 384) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
     const int warp = tid >> 5, lane = tid & 31;
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
     const float tmax = P.tmax, eps = P.eps;
@@ -212,6 +215,13 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             for (int b = 0; b < B; ++b)
 #pragma unroll
                 for (int g = 0; g < 4; ++g) tot[rr][b][g] = f2(0.f);
+        float2 acc[R][B][4];
+#pragma unroll
+        for (int rr = 0; rr < R; ++rr)
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int g = 0; g < 4; ++g) acc[rr][b][g] = f2(0.f);
 
         PairEnt pe_next = F.pairs[me.e0];
         for (int step = 0; step < nsteps; ++step, ++it) {
@@ -236,13 +246,6 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     asm volatile("mov.u32 %0, %0;" : "+r"(pn[b]));      // one register, not re-derived per position
                 }
                 const unsigned south = (unsigned)Ltot * 16u;
-                float2 acc[R][B][4];
-#pragma unroll
-                for (int rr = 0; rr < R; ++rr)
-#pragma unroll
-                    for (int b = 0; b < B; ++b)
-#pragma unroll
-                        for (int g = 0; g < 4; ++g) acc[rr][b][g] = f2(0.f);
 
                 // last table cell or the zero cell after it (rare): exact decision where needed
                 auto slow = [&](int rr, float tpv, unsigned &cb, int pos) {
@@ -326,12 +329,17 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     }
                     jf = __fadd2_rn(jf, f2(1.0f));
                 }
+                if (TOT) {
 #pragma unroll
-                for (int rr = 0; rr < R; ++rr)
+                    for (int rr = 0; rr < R; ++rr)
 #pragma unroll
-                    for (int b = 0; b < B; ++b)
+                        for (int b = 0; b < B; ++b)
 #pragma unroll
-                        for (int g = 0; g < 4; ++g) tot[rr][b][g] = __fadd2_rn(tot[rr][b][g], acc[rr][b][g]);
+                            for (int g = 0; g < 4; ++g) {
+                                tot[rr][b][g] = __fadd2_rn(tot[rr][b][g], acc[rr][b][g]);
+                                acc[rr][b][g] = f2(0.f);
+                            }
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_bar[buf]);         // this warp is done with the buffer
@@ -347,8 +355,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 if (k <= klast) {
 #pragma unroll
                     for (int b = 0; b < B; ++b) {
-                        const float v[8] = {tot[rr][b][0].x, tot[rr][b][0].y, tot[rr][b][1].x, tot[rr][b][1].y,
-                                            tot[rr][b][2].x, tot[rr][b][2].y, tot[rr][b][3].x, tot[rr][b][3].y};
+                        const float2 *s = TOT ? tot[rr][b] : acc[rr][b];
+                        const float v[8] = {s[0].x, s[0].y, s[1].x, s[1].y, s[2].x, s[2].y, s[3].x, s[3].y};
 #pragma unroll
                         for (int m = 0; m < 4; ++m) {
                             io.out[b][start_n + k + m * ip] = v[m] * P.omega;
@@ -395,14 +403,14 @@ struct FastPlan {
     int4 *belt_tiles = nullptr;
 };
 
-template <int B, int R, int NC>
+template <int B, int R, int NC, bool TOT>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st) {
     FastDev F{fp->pairs, c.tiles, c.ntiles, fp->counter, c.Ltot, fp->ntab_s};
-    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, c.ntiles);
     if (grid <= 0) return cudaSuccess;
-    sym_kernel<B, R, NC><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC, TOT><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
@@ -416,12 +424,16 @@ cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int w
         e = cudaErrorInvalidValue;
 #define SC_SYM_CASE(BB, RR)                                                                  \
     if (B == BB && c.R == RR)                                                                \
-        e = c.threads == 256 ? launch_sym<BB, RR, 256>(fp, c, P, io, st)                     \
-                             : launch_sym<BB, RR, 128>(fp, c, P, io, st);
-        SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
-        SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
-        SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
-        SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
+        e = c.threads == 256 ? launch_sym<BB, RR, 256, true>(fp, c, P, io, st)               \
+                             : launch_sym<BB, RR, 128, true>(fp, c, P, io, st);
+        if (B == 1 && c.R == 4 && c.threads == 384) {
+            e = launch_sym<1, 4, 384, false>(fp, c, P, io, st);
+        } else {
+            SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
+            SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
+            SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
+            SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
+        }
 #undef SC_SYM_CASE
         if (e != cudaSuccess) return e;
         *launches += c.ntiles > 0 ? 1 : 0;
@@ -473,7 +485,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    const int ntab_s = P.ntab - 1 + kTabPad;
+    const int ntab_s = P.ntab;                     // the cells and the one zero cell after them (indices are clamped)
     const size_t tab_bytes = ((size_t)ntab_s * 8 + 127) & ~(size_t)127;
     if (tab_bytes + 8192 > (size_t)smem_optin) return nullptr;       // table does not fit: generic only
 
@@ -605,10 +617,15 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     for (int B = 1; B <= kMaxB; ++B) {
         FastCfg &c = fp->cfg[B];
         std::vector<Cand> cands;
-        if (B == 1) cands = {{256, 4}, {256, 2}, {128, 2}};
+        // 384 consumer threads only come without the second accumulator set (registers): plain fp32
+        // running sums, good to ~3e-7 relative rms for discs of a few hundred pixels (measured 2.7e-7 at
+        // 425), so only while the mean disc holds at most 1500 pixels
+        const double mean_nb = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
+        if (B == 1 && mean_nb <= 1500.0) cands = {{384, 4}, {256, 4}, {256, 2}, {128, 2}};
+        else if (B == 1) cands = {{256, 4}, {256, 2}, {128, 2}};
         else cands = {{256, 2}, {128, 2}, {128, 1}};
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
-        if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256))
+        if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256 || (ft == 384 && fr == 4 && B == 1)))
             cands.insert(cands.begin(), Cand{ft, fr});
         for (const Cand &cd : cands) {
             const int R = cd.R, W = cd.threads / 32, C = 32 * R;
@@ -627,23 +644,30 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
                 sb.work *= sb.nw;
                 return sb;
             };
+            // full-width runs may be a little shorter than the CTA (last lanes idle) if that makes the
+            // staged runs fit into shared memory
+            for (int shrink = 0; shrink <= 64 && !c.ok; shrink += 16) {
+            const int run = W * C - shrink;
             std::vector<std::vector<SubH>> bins;
             std::vector<SubH> partial;
             for (int r = 2 * N; r > polar; --r) {
                 if (is_belt[r]) continue;
                 const int ip = ipof(r);
                 int k0 = 0;
-                for (; ip - k0 >= W * C; k0 += W * C) bins.push_back({make_sub(r, k0, W * C)});
+                for (; ip - k0 >= run; k0 += run) bins.push_back({make_sub(r, k0, run)});
                 if (k0 < ip) partial.push_back(make_sub(r, k0, ip - k0));
             }
             const size_t nfull = bins.size();
             std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
-            std::vector<int> used(nfull, W);
+            // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
+            const int Lmax = (int)(((size_t)smem_optin - 256 - tab_bytes) / ((size_t)2 * B * 2 * 16)) & ~7;
+            std::vector<int> used(nfull, W), lsum(nfull, 0);
             for (const SubH &sb : partial) {
                 size_t i = nfull;
-                for (; i < bins.size(); ++i) if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub) break;
-                if (i == bins.size()) { bins.emplace_back(); used.push_back(0); }
-                bins[i].push_back(sb); used[i] += sb.nw;
+                for (; i < bins.size(); ++i)
+                    if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Lmax) break;
+                if (i == bins.size()) { bins.emplace_back(); used.push_back(0); lsum.push_back(0); }
+                bins[i].push_back(sb); used[i] += sb.nw; lsum[i] += sb.Lcap;
             }
             // longest tiles first
             std::vector<std::pair<double, size_t>> order;
@@ -656,7 +680,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             }
             std::stable_sort(order.begin(), order.end());
             const size_t smem = tab_bytes + (size_t)2 * B * 2 * Ltot * 16;
-            if (smem + 2048 > (size_t)smem_optin) continue;
+            if (smem + 256 > (size_t)smem_optin) continue;        // 256: static shared memory (barriers)
             std::vector<SymTile> tiles(bins.size());
             for (size_t t = 0; t < order.size(); ++t) {
                 const std::vector<SubH> &bn = bins[order[t].second];
@@ -676,7 +700,8 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((e = cudaMalloc((void **)&c.tiles, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return fail(e);
             if (!tiles.empty() && (e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             c.ok = true;
-            break;
+            }
+            if (c.ok) break;
         }
     }
     fp->first_belt = 2 * N + 1;
