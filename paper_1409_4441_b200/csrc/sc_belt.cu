@@ -25,7 +25,6 @@ namespace sc {
 constexpr int kBeltProd = 128;   // producer threads: warp 0 of them issues TMA, warps 1-3 evaluate taps
 constexpr int kTapThreads = 96;
 constexpr int kMaxBuf = 4;
-constexpr int kBeltSlack = 256;  // floats per staged plane beyond the tile: window + alignment
 
 static __device__ __noinline__ unsigned belt_exact_mask(const Dev &P, int r, int k, int rq, int kq) {
     const int N = P.nside, N4 = 4 * N;
@@ -81,10 +80,12 @@ __device__ __forceinline__ void belt_window(const PairEnt &pe, int sh, int k0, i
     ng = (2 * pe.hw + 4 + a0 + 3) >> 2;
 }
 
-template <int NC>
+// SLACK: floats per staged plane beyond the tile (window + alignment); TOT: second accumulator set
+// (flushed every >= 48 taps; needed for discs of thousands of pixels, costs 32 registers).
+template <int NC, int SLACK, bool TOT>
 __global__ void __launch_bounds__(NC + kBeltProd, 1)
 belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
-    constexpr int T = 4 * NC, LP = T + kBeltSlack;
+    constexpr int T = 4 * NC, LP = T + SLACK;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int N = P.nside, N4 = 4 * N;
@@ -105,6 +106,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
 
     if (tid >= NC) {
         if (NC == 256) asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+        if (NC == 512) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
         if (tid < NC + 32) {
             // ================================ TMA producer warp ================================
             int buf = 0; unsigned par = 0;
@@ -202,6 +204,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
 
     // ==================================== consumers ====================================
     if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+    if (NC == 512) asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
     int buf = 0; unsigned par = 0;
     int tb = 0; unsigned tpar = 0;
     for (int row = 0; row < nrows; ++row) {
@@ -277,7 +280,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
                 if (++buf == NBUF) { buf = 0; par ^= 1u; }
                 ntaps += d.z;
-                if (ntaps >= 48 || e + 1 == ne) {
+                if (TOT && (ntaps >= 48 || e + 1 == ne)) {
 #pragma unroll
                     for (int g = 0; g < 8; ++g) {
                         tot01[g] = __fadd2_rn(tot01[g], acc01[g]); tot23[g] = __fadd2_rn(tot23[g], acc23[g]);
@@ -287,6 +290,10 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 }
             }
 
+            if (!TOT) {
+#pragma unroll
+                for (int g = 0; g < 8; ++g) { tot01[g] = acc01[g]; tot23[g] = acc23[g]; }
+            }
             // ---- uncertain taps: canonical fp64 decision per pixel pair and image ------------------
             if (nexc > 0) {
                 float tt[4][8];
@@ -348,24 +355,26 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
 }
 
 // host ------------------------------------------------------------------------------------------
-size_t belt_smem_bytes(int NC, int nbuf, int ntb, int pw_max, int ne_max) {
-    return (size_t)nbuf * 8 * (4 * NC + kBeltSlack) * 4 + (size_t)ntb * TapLayout(pw_max, ne_max).bytes;
+size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_max) {
+    return (size_t)nbuf * 8 * (4 * NC + slack) * 4 + (size_t)ntb * TapLayout(pw_max, ne_max).bytes;
 }
-int belt_max_chunk_floats() { return kBeltSlack + 4; }                   // 4 ng may not exceed this
 
-template <int NC>
+template <int NC, int SLACK, bool TOT>
 static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io, int B, size_t smem, int nsm, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(belt_kernel<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(belt_kernel<NC, SLACK, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int grid = F.ntiles < nsm ? F.ntiles : nsm;
-    belt_kernel<NC><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
+    belt_kernel<NC, SLACK, TOT><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
     return cudaGetLastError();
 }
 
+// variants: (512 consumer threads, slack 64, single accumulator set) for small discs on Nside % 2048 == 0;
+// (256 | 128, slack 256, two accumulator sets) otherwise
 cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
                         cudaStream_t st) {
-    if (threads == 256) return launch_belt_nc<256>(P, F, io, B, smem, nsm, st);
-    if (threads == 128) return launch_belt_nc<128>(P, F, io, B, smem, nsm, st);
+    if (threads == 512) return launch_belt_nc<512, 64, false>(P, F, io, B, smem, nsm, st);
+    if (threads == 256) return launch_belt_nc<256, 256, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 128) return launch_belt_nc<128, 256, true>(P, F, io, B, smem, nsm, st);
     return cudaErrorInvalidValue;
 }
 

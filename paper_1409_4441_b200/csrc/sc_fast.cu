@@ -372,8 +372,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-size_t belt_smem_bytes(int NC, int nbuf, int ntb, int pw_max, int ne_max);
-int belt_max_chunk_floats();
+size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_max);
 cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
                         cudaStream_t st);
 
@@ -563,13 +562,24 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     // ---- belt kernel: base rings whose input rings all have 4N pixels ------------------------------
     std::vector<char> is_belt(2 * N + 1, 0);
     const bool no_belt = std::getenv("SC_NO_BELT") != nullptr;
-    const int bNC = (N % 1024 == 0) ? 256 : (N % 512 == 0 ? 128 : 0);       // consumer threads, tile = 4 bNC pixels
-    if (!no_belt && bNC) {
+    // variants (consumer threads, slack floats per plane): tile = 4 x threads base pixels, must divide N
+    struct BeltVar { int nc, slack; };
+    std::vector<BeltVar> bvars;
+    {
+        const double mean_nb_b = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
+        if (N % 2048 == 0 && mean_nb_b <= 1500.0 && !std::getenv("SC_BELT_NO512")) bvars.push_back({512, 64});
+        if (N % 1024 == 0) bvars.push_back({256, 256});
+        else if (N % 512 == 0) bvars.push_back({128, 256});
+    }
+    for (const BeltVar &bv : bvars) {
+        if (no_belt || fp->belt_ok) break;
+        const int bNC = bv.nc;
         const int T = 4 * bNC;
         std::vector<int> woff(pairs.size(), 0);
         std::vector<int4> btiles;
         int pw_max = 0, ne_max = 0;
         bool fits = true;
+        std::fill(is_belt.begin(), is_belt.end(), 0);
         for (int r = 2 * N; r > polar; --r) {
             if (ipof(r) != N) continue;
             bool all = true;
@@ -580,7 +590,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int base = pair_off[slot_of[r]];
             for (size_t i = 0; i < per_ring[r].size(); ++i) {
                 const int ng_max = (2 * per_ring[r][i].hw + 4 + 3 + 3) >> 2;   // chunks of 4 staged positions
-                if (4 * ng_max > belt_max_chunk_floats()) fits = false;
+                if (4 * ng_max > bv.slack + 4) fits = false;                    // plane = T - 4 + 4 ng floats
                 woff[base + i] = off;
                 off += (4 * ng_max + 2 + 1) & ~1;                              // tap pairs, even count
             }
@@ -593,11 +603,11 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         if (fits && !btiles.empty()) {
             const int combos[6][2] = {{2, 4}, {2, 3}, {1, 4}, {2, 2}, {1, 3}, {1, 2}};       // (tap buffers, stage buffers)
             for (const auto &cb : combos) {
-                bsmem = belt_smem_bytes(bNC, cb[1], cb[0], pw_max, ne_max);
+                bsmem = belt_smem_bytes(bNC, bv.slack, cb[1], cb[0], pw_max, ne_max);
                 if (bsmem + 2048 <= (size_t)smem_optin) { ntb = cb[0]; nbuf = cb[1]; break; }
             }
         }
-        if (nbuf) {
+        if (nbuf >= (bNC == 512 ? 3 : 2)) {
             if ((e = cudaMalloc((void **)&fp->woff, woff.size() * sizeof(int))) != cudaSuccess) return fail(e);
             if ((e = cudaMemcpy(fp->woff, woff.data(), woff.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
