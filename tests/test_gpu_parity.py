@@ -254,6 +254,39 @@ def test_batch_chunking_and_host_entry(sc):
         _check_values(batch[b], ref[b], f"batch6 map{b}")
 
 
+@pytest.mark.parametrize("nside,theta_deg,ntab,B", [(512, 1.0, 4096, 1),      # belt_kernel<128>, sym 384 variant
+                                                   (512, 2.5, 2048, 2),      # belt_kernel<128>, B = 2, two accumulator sets
+                                                   (768, 0.8, 4096, 1),      # Nside not a multiple of 512: no belt kernel
+                                                   (1024, 1.2, 8192, 1)])    # belt_kernel<256>, discs of ~1500 pixels
+def test_other_kernel_variants_sampled(sc, nside, theta_deg, ntab, B):
+    """Shapes outside BASELINE.json's five configs that select the other kernel variants: sampled pixels
+    (poles, cap/belt boundaries, equator + random) and whole rings around the kernel boundaries."""
+    theta = theta_deg * gen.DEG
+    npix = 12 * nside * nside
+    _, th = gen.table_nodes(theta, ntab)
+    T = np.exp(-3.0 * (th / theta) ** 2) * np.cos(4.0 * th / theta) + 0.05
+    maps = [gen.noise_map(npix, 300 + nside + b) for b in range(B)]
+    tb = O.ring_table(nside)
+    with sc.Plan(nside, T, theta, B) as plan:
+        part = plan.partition()
+        pr, fb = part["polar_rings"], part["first_belt_ring"]
+        rings = sorted({1, 2, pr, pr + 1, nside - 1, nside, nside + 1, min(fb, 2 * nside) - 1, min(fb, 2 * nside),
+                        2 * nside - 1, 2 * nside, 2 * nside + 1, 4 * nside - min(fb, 2 * nside), 4 * nside - pr,
+                        4 * nside - pr - 1, 4 * nside - 1} - {0})
+        sel = np.concatenate([np.arange(tb["start"][r - 1], tb["start"][r - 1] + tb["npr"][r - 1]) for r in rings]
+                             + [gen.sample_pixels(nside, 3000, seed=nside)])
+        sel = np.unique(sel)
+        ref, cnt, sig = O.convolve(nside, T, theta, maps, sel=sel)
+        c, s = plan.neighbour_counts()
+        c, s = c.cpu().numpy(), s.cpu().numpy().view(np.uint64)
+        np.testing.assert_array_equal(c[sel], cnt)
+        np.testing.assert_array_equal(s[sel], sig)
+        out = _gpu_convolve(sc, plan, maps)
+        for b in range(B):
+            _check_values(out[b][sel], ref[b], f"nside {nside} theta {theta_deg} B {B} map{b} {part}")
+            assert np.all(np.isfinite(out[b]))
+
+
 def test_profile_entry_and_partition(sc):
     """sc_convolve_profile runs the same launches as sc_convolve (bit-identical output) and reports a
     positive device time for every kernel the plan uses; sc_plan_partition is consistent with them."""
