@@ -68,6 +68,8 @@ __device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
 
 constexpr int kSymProd = 128;     // producer threads per CTA (one warpgroup): they only issue cp.async
 constexpr int kSymBuf = 2;        // stage buffers
+constexpr int kSymChunksDflt = 5;  // latitude chunks of the cap rings for the pipelined host entry
+constexpr int kBeltChunksDflt = 6; // same for the belt rings
 
 // Tile n of this CTA: rows of gridDim.x tiles, alternate rows reversed ("snake") so that the CTAs
 // get equal shares of the work-sorted tile list without a global counter.
@@ -380,8 +382,9 @@ struct FastCfg {            // per batch size
     bool ok = false;
     int threads = 0, R = 1, Ltot = 0;
     size_t smem = 0;
-    SymTile *tiles = nullptr;
-    int ntiles = 0;
+    SymTile *tiles = nullptr;     // [0, ntiles): all rings, work sorted; then the latitude chunks
+    int ntiles = 0, ntiles_all = 0;
+    std::vector<int> ch_off, ch_lo, ch_hi;   // chunk i: tiles [ch_off[i], ch_off[i+1]), base rings ch_lo[i] .. ch_hi[i]
 };
 
 struct FastPlan {
@@ -400,33 +403,42 @@ struct FastPlan {
     int *pair_off = nullptr;
     int *woff = nullptr;
     int4 *belt_tiles = nullptr;
+    std::vector<int> bch_off, bch_lo, bch_hi;   // belt latitude chunks (tile offsets, base rings), equator first
 };
 
 template <int B, int R, int NC, bool TOT>
-static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st) {
-    FastDev F{fp->pairs, c.tiles, c.ntiles, fp->counter, c.Ltot, fp->ntab_s};
+static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st,
+                              int t0, int nt) {
+    FastDev F{fp->pairs, c.tiles + t0, nt, fp->counter, c.Ltot, fp->ntab_s};
     cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
-    const int grid = std::min(fp->nsm, c.ntiles);
+    const int grid = std::min(fp->nsm, nt);
     if (grid <= 0) return cudaSuccess;
     sym_kernel<B, R, NC, TOT><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
-// which: bit 0 = sym kernel, bit 1 = belt kernel (the two write disjoint pixels and may run on different streams)
-cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches) {
+// which: bit 0 = sym kernel, bit 1 = belt kernel (the two write disjoint pixels and may run on different
+// streams); chunk < 0: all tiles (work sorted), else latitude chunk `chunk` of that kernel
+cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches,
+                        int chunk) {
     *launches = 0;
     if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return cudaErrorInvalidValue;
     const FastCfg &c = fp->cfg[B];
     cudaError_t e = cudaSuccess;
     if (which & 1) {
+        int t0 = 0, nt = c.ntiles;
+        if (chunk >= 0) {
+            if (chunk + 1 >= (int)c.ch_off.size()) return cudaErrorInvalidValue;
+            t0 = c.ch_off[chunk]; nt = c.ch_off[chunk + 1] - t0;
+        }
         e = cudaErrorInvalidValue;
 #define SC_SYM_CASE(BB, RR)                                                                  \
     if (B == BB && c.R == RR)                                                                \
-        e = c.threads == 256 ? launch_sym<BB, RR, 256, true>(fp, c, P, io, st)               \
-                             : launch_sym<BB, RR, 128, true>(fp, c, P, io, st);
+        e = c.threads == 256 ? launch_sym<BB, RR, 256, true>(fp, c, P, io, st, t0, nt)       \
+                             : launch_sym<BB, RR, 128, true>(fp, c, P, io, st, t0, nt);
         if (B == 1 && c.R == 4 && c.threads == 384) {
-            e = launch_sym<1, 4, 384, false>(fp, c, P, io, st);
+            e = launch_sym<1, 4, 384, false>(fp, c, P, io, st, t0, nt);
         } else {
             SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
             SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
@@ -435,23 +447,40 @@ cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int w
         }
 #undef SC_SYM_CASE
         if (e != cudaSuccess) return e;
-        *launches += c.ntiles > 0 ? 1 : 0;
+        *launches += nt > 0 ? 1 : 0;
     }
     if ((which & 2) && fp->belt_ok) {
-        e = launch_belt(P, fp->belt, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
-        if (e == cudaSuccess) ++*launches;
+        BeltDev F = fp->belt;
+        if (chunk >= 0) {
+            if (chunk + 1 >= (int)fp->bch_off.size()) return cudaErrorInvalidValue;
+            F.tiles += fp->bch_off[chunk]; F.ntiles = fp->bch_off[chunk + 1] - fp->bch_off[chunk];
+        }
+        if (F.ntiles > 0) {
+            e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
+            if (e == cudaSuccess) ++*launches;
+        }
     }
     return e;
+}
+
+// latitude chunks for the pipelined host entry: kind 0 = sym kernel, 1 = belt kernel
+int fast_chunk_count(const FastPlan *fp, int B, int kind) {
+    if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return 0;
+    return kind == 0 ? (int)fp->cfg[B].ch_lo.size() : (fp->belt_ok ? (int)fp->bch_lo.size() : 0);
+}
+void fast_chunk_rings(const FastPlan *fp, int B, int kind, int i, int *lo, int *hi) {
+    if (kind == 0) { *lo = fp->cfg[B].ch_lo[i]; *hi = fp->cfg[B].ch_hi[i]; }
+    else { *lo = fp->bch_lo[i]; *hi = fp->bch_hi[i]; }
 }
 
 cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches,
                           cudaEvent_t *ev) {
     int n1 = 0, n2 = 0;
-    cudaError_t e = fast_launch(fp, P, io, B, 1, st, &n1);
+    cudaError_t e = fast_launch(fp, P, io, B, 1, st, &n1, -1);
     *launches = n1;
     if (e != cudaSuccess) return e;
     if (ev && (e = cudaEventRecord(ev[0], st)) != cudaSuccess) return e;      // end of the sym kernel
-    e = fast_launch(fp, P, io, B, 2, st, &n2);
+    e = fast_launch(fp, P, io, B, 2, st, &n2, -1);
     *launches += n2;
     if (ev && e == cudaSuccess) e = cudaEventRecord(ev[1], st);              // end of the belt kernel
     return e;
@@ -614,6 +643,23 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((e = cudaMemcpy(fp->belt_tiles, btiles.data(), btiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, (int)btiles.size(), pw_max, ne_max, nbuf, ntb};
             fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true;
+            // latitude chunks: the tile list runs from ring 2N down to the first belt ring, N / T tiles per ring
+            {
+                int r_first = 2 * N + 1;
+                for (int r = 2 * N; r > polar && is_belt[r]; --r) r_first = r;
+                const int nrings = 2 * N - r_first + 1, per_ring_tiles = N / T;
+                fp->bch_off.assign(1, 0); fp->bch_lo.clear(); fp->bch_hi.clear();
+                int hi = 2 * N;
+                const int nbch = std::max(1, env_int("SC_BELT_CHUNKS", kBeltChunksDflt));
+                for (int cidx = 1; cidx <= nbch && hi >= r_first; ++cidx) {
+                    int lo = 2 * N + 1 - (int)((long long)nrings * cidx / nbch);
+                    if (cidx == nbch) lo = r_first;
+                    if (lo > hi) continue;
+                    fp->bch_lo.push_back(lo); fp->bch_hi.push_back(hi);
+                    fp->bch_off.push_back((2 * N - lo + 1) * per_ring_tiles);
+                    hi = lo - 1;
+                }
+            }
         } else {
             std::fill(is_belt.begin(), is_belt.end(), 0);
         }
@@ -658,55 +704,81 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             // staged runs fit into shared memory
             for (int shrink = 0; shrink <= 64 && !c.ok; shrink += 16) {
             const int run = W * C - shrink;
-            std::vector<std::vector<SubH>> bins;
-            std::vector<SubH> partial;
-            for (int r = 2 * N; r > polar; --r) {
-                if (is_belt[r]) continue;
-                const int ip = ipof(r);
-                int k0 = 0;
-                for (; ip - k0 >= run; k0 += run) bins.push_back({make_sub(r, k0, run)});
-                if (k0 < ip) partial.push_back(make_sub(r, k0, ip - k0));
-            }
-            const size_t nfull = bins.size();
-            std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int Lmax = (int)(((size_t)smem_optin - 256 - tab_bytes) / ((size_t)2 * B * 2 * 16)) & ~7;
-            std::vector<int> used(nfull, W), lsum(nfull, 0);
-            for (const SubH &sb : partial) {
-                size_t i = nfull;
-                for (; i < bins.size(); ++i)
-                    if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Lmax) break;
-                if (i == bins.size()) { bins.emplace_back(); used.push_back(0); lsum.push_back(0); }
-                bins[i].push_back(sb); used[i] += sb.nw; lsum[i] += sb.Lcap;
-            }
-            // longest tiles first
-            std::vector<std::pair<double, size_t>> order;
-            int Ltot = 0;
-            for (size_t i = 0; i < bins.size(); ++i) {
-                double w = 0; int L = 0;
-                for (const SubH &sb : bins[i]) { w = std::max(w, sb.work / sb.nw); L += sb.Lcap; }
-                order.push_back({-w, i});
-                Ltot = std::max(Ltot, L);
-            }
-            std::stable_sort(order.begin(), order.end());
-            const size_t smem = tab_bytes + (size_t)2 * B * 2 * Ltot * 16;
-            if (smem + 256 > (size_t)smem_optin) continue;        // 256: static shared memory (barriers)
-            std::vector<SymTile> tiles(bins.size());
-            for (size_t t = 0; t < order.size(); ++t) {
-                const std::vector<SubH> &bn = bins[order[t].second];
-                SymTile &tl = tiles[t];
-                std::memset(&tl, 0, sizeof(tl));
-                tl.nsub = (int)bn.size();
-                int w0 = 0, soff = 0;
-                for (int i = 0; i < tl.nsub; ++i) {
-                    const SubH &sb = bn[i];
-                    const int slot = slot_of[sb.r];
-                    tl.sub[i] = SubTile{sb.r, sb.k0, sb.n, pair_off[slot], pair_off[slot + 1] - pair_off[slot], w0, sb.nw, soff};
-                    tl.nsteps = std::max(tl.nsteps, tl.sub[i].ne);
-                    w0 += sb.nw; soff += sb.Lcap;
+            // tiles of the non-belt base rings r_lo .. r_hi, longest first; returns the staged positions needed
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tiles) -> int {
+                std::vector<std::vector<SubH>> bins;
+                std::vector<SubH> partial;
+                for (int r = r_hi; r >= r_lo; --r) {
+                    if (is_belt[r]) continue;
+                    const int ip = ipof(r);
+                    int k0 = 0;
+                    for (; ip - k0 >= run; k0 += run) bins.push_back({make_sub(r, k0, run)});
+                    if (k0 < ip) partial.push_back(make_sub(r, k0, ip - k0));
+                }
+                const size_t nfull = bins.size();
+                std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
+                std::vector<int> used(nfull, W), lsum(nfull, 0);
+                for (const SubH &sb : partial) {
+                    size_t i = nfull;
+                    for (; i < bins.size(); ++i)
+                        if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Lmax) break;
+                    if (i == bins.size()) { bins.emplace_back(); used.push_back(0); lsum.push_back(0); }
+                    bins[i].push_back(sb); used[i] += sb.nw; lsum[i] += sb.Lcap;
+                }
+                std::vector<std::pair<double, size_t>> order;
+                int Lneed = 0;
+                for (size_t i = 0; i < bins.size(); ++i) {
+                    double w = 0; int L = 0;
+                    for (const SubH &sb : bins[i]) { w = std::max(w, sb.work / sb.nw); L += sb.Lcap; }
+                    order.push_back({-w, i});
+                    Lneed = std::max(Lneed, L);
+                }
+                std::stable_sort(order.begin(), order.end());
+                const size_t t0 = tiles.size();
+                tiles.resize(t0 + bins.size());
+                for (size_t t = 0; t < order.size(); ++t) {
+                    const std::vector<SubH> &bn = bins[order[t].second];
+                    SymTile &tl = tiles[t0 + t];
+                    std::memset(&tl, 0, sizeof(tl));
+                    tl.nsub = (int)bn.size();
+                    int w0 = 0, soff = 0;
+                    for (int i = 0; i < tl.nsub; ++i) {
+                        const SubH &sb = bn[i];
+                        const int slot = slot_of[sb.r];
+                        tl.sub[i] = SubTile{sb.r, sb.k0, sb.n, pair_off[slot], pair_off[slot + 1] - pair_off[slot], w0, sb.nw, soff};
+                        tl.nsteps = std::max(tl.nsteps, tl.sub[i].ne);
+                        w0 += sb.nw; soff += sb.Lcap;
+                    }
+                }
+                return Lneed;
+            };
+            // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
+            // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
+            std::vector<SymTile> tiles;
+            int Ltot = build(2 * N, polar + 1, tiles);
+            int sym_hi = 2 * N;
+            while (sym_hi > polar && is_belt[sym_hi]) --sym_hi;
+            std::vector<int> ch_off(1, (int)tiles.size()), ch_lo, ch_hi;
+            {
+                const long long nsymch = std::max(1, env_int("SC_SYM_CHUNKS", kSymChunksDflt));
+                long long total_px = 0, acc_px = 0;
+                for (int r = sym_hi; r > polar; --r) total_px += ipof(r);
+                int hi = sym_hi, nch = 0;
+                for (int r = sym_hi; r > polar; --r) {
+                    acc_px += ipof(r);
+                    if (r == polar + 1 || acc_px * nsymch >= total_px * (nch + 1)) {
+                        Ltot = std::max(Ltot, build(hi, r, tiles));
+                        ch_off.push_back((int)tiles.size()); ch_lo.push_back(r); ch_hi.push_back(hi);
+                        hi = r - 1; ++nch;
+                    }
                 }
             }
-            c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = (int)tiles.size();
+            const size_t smem = tab_bytes + (size_t)2 * B * 2 * Ltot * 16;
+            if (smem + 256 > (size_t)smem_optin) continue;        // 256: static shared memory (barriers)
+            c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
+            c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all;
             if ((e = cudaMalloc((void **)&c.tiles, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return fail(e);
             if (!tiles.empty() && (e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             c.ok = true;

@@ -22,7 +22,9 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
 void fast_plan_destroy(FastPlan *fp);
 cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cudaStream_t st, int *launches, cudaEvent_t *ev);
 int fast_first_belt_ring(const FastPlan *fp);
-cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches);
+cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches, int chunk);
+int fast_chunk_count(const FastPlan *fp, int B, int kind);
+void fast_chunk_rings(const FastPlan *fp, int B, int kind, int i, int *lo, int *hi);
 bool fast_available(const FastPlan *fp, int B);
 }  // namespace sc
 
@@ -89,7 +91,8 @@ struct sc_plan {
     float *stage_in = nullptr, *stage_out = nullptr;
     int stage_maps = 0;
     cudaStream_t own_stream = nullptr, comp_stream = nullptr, d2h_stream = nullptr;
-    cudaEvent_t ev_belt_in = nullptr, ev_all_in = nullptr, ev_belt_done = nullptr, ev_rest_done = nullptr, ev_prev = nullptr;
+    std::vector<cudaEvent_t> events;           // pool for the pipelined host entry
+    std::vector<int> rlo_h;                    // host copy of the first candidate input ring of every ring
     mutable int last_launches = 0;
     sc::FastPlan *fast = nullptr;
     int polar_rings = 0;                       // rings 1..polar_rings and their southern mirrors use the generic kernel
@@ -259,6 +262,7 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
             if (hi < nr) ++hi;
             rlo[i - 1] = lo; rhi[i - 1] = hi;
         }
+        pl->rlo_h = rlo;
         // device table in the reversed coordinate t = (1 - x) (n-1)/(1-c): node j of the device
         // table is caller node n-1-j.  Cell [j, j+1): K = a_j + t b_j with b_j = T'_{j+1} - T'_j,
         // a_j = T'_j - j b_j  (fp64, rounded once).  Zero padding after the last cell.
@@ -303,8 +307,7 @@ sc_status sc_plan_destroy(sc_plan *plan) {
     if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
     if (plan->comp_stream) cudaStreamDestroy(plan->comp_stream);
     if (plan->d2h_stream) cudaStreamDestroy(plan->d2h_stream);
-    for (cudaEvent_t e : {plan->ev_belt_in, plan->ev_all_in, plan->ev_belt_done, plan->ev_rest_done, plan->ev_prev})
-        if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : plan->events) cudaEventDestroy(e);
     delete plan;
     return SC_OK;
 }
@@ -424,8 +427,7 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
     if (!plan->own_stream) SC_CUDA(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
     const sc::Dev &D = plan->dev;
     const int N = D.nside;
-    const int fb = plan->fast ? sc::fast_first_belt_ring(plan->fast) : 2 * N + 1;
-    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && fb <= 2 * N;
+    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && sc::fast_available(plan->fast, std::min(B, sc::kMaxB));
     if (!pipelined) {
         std::vector<const float *> in(B); std::vector<float *> out(B);
         for (int b = 0; b < B; ++b) {
@@ -440,55 +442,87 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
         return SC_OK;
     }
 
-    // Pipelined: the belt kernel reads only belt rings (N .. 3N) and writes base rings fb .. 2N and
-    // their mirrors, so it can start as soon as the belt rows have arrived and its output can travel
-    // back while the cap kernels still run.  Three streams (copy in, compute, copy out) and events.
+    // Pipelined over latitude chunks, from the equator towards the poles: a chunk of base rings lo .. hi
+    // (and their southern mirrors) needs the input rows of rings rlo(lo) .. 4N - rlo(lo), one contiguous
+    // range that grows outwards, so the copy-in stream sends two new slices per chunk, the compute
+    // stream runs the chunk's tiles as soon as they have arrived, and the copy-out stream returns the
+    // chunk's output rows while later chunks are still being copied in and computed.
     if (!plan->comp_stream) {
         SC_CUDA(cudaStreamCreateWithFlags(&plan->comp_stream, cudaStreamNonBlocking));
         SC_CUDA(cudaStreamCreateWithFlags(&plan->d2h_stream, cudaStreamNonBlocking));
-        for (cudaEvent_t *e : {&plan->ev_belt_in, &plan->ev_all_in, &plan->ev_belt_done, &plan->ev_rest_done, &plan->ev_prev})
-            SC_CUDA(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
     }
     cudaStream_t s_in = plan->own_stream, s_c = plan->comp_stream, s_out = plan->d2h_stream;
-    const size_t belt_lo = (size_t)D.ncap, belt_hi = npix - (size_t)D.ncap;                 // input rows of the belt kernel
-    const size_t ob_lo = (size_t)plan->rings[fb - 1].start;                                // its output rows
-    const size_t ob_hi = (4 * N - fb + 1 <= 4 * N - 1) ? (size_t)plan->rings[4 * N - fb].start : npix;
+    const int N4 = 4 * N;
+    auto row = [&](int ring) -> size_t { return ring <= N4 - 1 ? (size_t)plan->rings[ring - 1].start : npix; };   // first pixel of a ring
     const int pr = plan->polar_rings;
     int launches = 0;
+    size_t nev = 0;
+    auto next_event = [&](cudaEvent_t *ev) -> sc_status {
+        if (nev == plan->events.size()) {
+            cudaEvent_t e = nullptr;
+            SC_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            plan->events.push_back(e);
+        }
+        *ev = plan->events[nev++];
+        return SC_OK;
+    };
     for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
         const int nb = std::min(sc::kMaxB, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = plan->stage_in + npix * (b0 + b); io.out[b] = plan->stage_out + npix * (b0 + b); }
-        for (int b = 0; b < nb; ++b)
-            SC_CUDA(cudaMemcpyAsync((float *)io.in[b] + belt_lo, in_maps_host[b0 + b] + belt_lo, (belt_hi - belt_lo) * 4, cudaMemcpyHostToDevice, s_in));
-        SC_CUDA(cudaEventRecord(plan->ev_belt_in, s_in));
-        for (int b = 0; b < nb; ++b) {
-            SC_CUDA(cudaMemcpyAsync((float *)io.in[b], in_maps_host[b0 + b], belt_lo * 4, cudaMemcpyHostToDevice, s_in));
-            SC_CUDA(cudaMemcpyAsync((float *)io.in[b] + belt_hi, in_maps_host[b0 + b] + belt_hi, (npix - belt_hi) * 4, cudaMemcpyHostToDevice, s_in));
+        auto copy_in = [&](size_t p0, size_t p1) -> sc_status {
+            for (int b = 0; b < nb && p1 > p0; ++b)
+                SC_CUDA(cudaMemcpyAsync((float *)io.in[b] + p0, in_maps_host[b0 + b] + p0, (p1 - p0) * 4, cudaMemcpyHostToDevice, s_in));
+            return SC_OK;
+        };
+        auto copy_out = [&](size_t p0, size_t p1) -> sc_status {
+            for (int b = 0; b < nb && p1 > p0; ++b)
+                SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b] + p0, io.out[b] + p0, (p1 - p0) * 4, cudaMemcpyDeviceToHost, s_out));
+            return SC_OK;
+        };
+        int have_lo = 2 * N + 1;                       // rows of rings have_lo .. 4N - have_lo are on the device
+        // stage: bring rows down to ring need_lo, launch, return rows of base rings lo .. hi
+        auto stage = [&](int need_lo, int kind, int chunk, int lo, int hi) -> sc_status {
+            sc_status s;
+            need_lo = std::max(1, std::min(need_lo, 2 * N));
+            if (need_lo < have_lo) {
+                if (have_lo > 2 * N) {
+                    if ((s = copy_in(row(need_lo), row(N4 - need_lo + 1))) != SC_OK) return s;
+                } else {
+                    if ((s = copy_in(row(need_lo), row(have_lo))) != SC_OK) return s;
+                    if ((s = copy_in(row(N4 - have_lo + 1), row(N4 - need_lo + 1))) != SC_OK) return s;
+                }
+                have_lo = need_lo;
+            }
+            cudaEvent_t ev_in, ev_done;
+            if ((s = next_event(&ev_in)) != SC_OK || (s = next_event(&ev_done)) != SC_OK) return s;
+            SC_CUDA(cudaEventRecord(ev_in, s_in));
+            SC_CUDA(cudaStreamWaitEvent(s_c, ev_in, 0));
+            int nl = 0;
+            if (kind == 2) {
+                const int np = 2 * pr * (pr + 1);
+                SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, s_c));
+                nl = 1;
+            } else {
+                SC_CUDA(sc::fast_launch(plan->fast, D, io, nb, kind == 0 ? 1 : 2, s_c, &nl, chunk));
+            }
+            launches += nl;
+            SC_CUDA(cudaEventRecord(ev_done, s_c));
+            SC_CUDA(cudaStreamWaitEvent(s_out, ev_done, 0));
+            if (hi >= 2 * N) return copy_out(row(lo), row(N4 - lo + 1));
+            if ((s = copy_out(row(lo), row(hi + 1))) != SC_OK) return s;
+            return copy_out(row(N4 - hi), row(N4 - lo + 1));
+        };
+        for (int kind = 1; kind >= 0; --kind) {        // belt chunks (equator first), then the cap chunks
+            const int nch = sc::fast_chunk_count(plan->fast, nb, kind);
+            for (int i = 0; i < nch; ++i) {
+                int lo, hi;
+                sc::fast_chunk_rings(plan->fast, nb, kind, i, &lo, &hi);
+                sc_status s = stage(plan->rlo_h[lo - 1] - 1, kind, i, lo, hi);
+                if (s != SC_OK) return s;
+            }
         }
-        SC_CUDA(cudaEventRecord(plan->ev_all_in, s_in));
-
-        int nl = 0;
-        SC_CUDA(cudaStreamWaitEvent(s_c, plan->ev_belt_in, 0));
-        SC_CUDA(sc::fast_launch(plan->fast, D, io, nb, 2, s_c, &nl)); launches += nl;
-        SC_CUDA(cudaEventRecord(plan->ev_belt_done, s_c));
-        SC_CUDA(cudaStreamWaitEvent(s_c, plan->ev_all_in, 0));
-        if (pr > 0) {
-            const int np = 2 * pr * (pr + 1);
-            SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, s_c));
-            ++launches;
-        }
-        SC_CUDA(sc::fast_launch(plan->fast, D, io, nb, 1, s_c, &nl)); launches += nl;
-        SC_CUDA(cudaEventRecord(plan->ev_rest_done, s_c));
-
-        SC_CUDA(cudaStreamWaitEvent(s_out, plan->ev_belt_done, 0));
-        for (int b = 0; b < nb; ++b)
-            SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b] + ob_lo, io.out[b] + ob_lo, (ob_hi - ob_lo) * 4, cudaMemcpyDeviceToHost, s_out));
-        SC_CUDA(cudaStreamWaitEvent(s_out, plan->ev_rest_done, 0));
-        for (int b = 0; b < nb; ++b) {
-            SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b], io.out[b], ob_lo * 4, cudaMemcpyDeviceToHost, s_out));
-            SC_CUDA(cudaMemcpyAsync(out_maps_host[b0 + b] + ob_hi, io.out[b] + ob_hi, (npix - ob_hi) * 4, cudaMemcpyDeviceToHost, s_out));
-        }
+        if (pr > 0) { sc_status s = stage(1, 2, 0, 1, pr); if (s != SC_OK) return s; }
     }
     plan->last_launches = launches;
     SC_CUDA(cudaStreamSynchronize(s_out));
