@@ -153,6 +153,29 @@ sc_status sc_convolve_profile(const sc_plan *plan, const float *const *in_maps,
  */
 sc_status sc_plan_partition(const sc_plan *plan, int *polar_rings, int *first_belt_ring);
 
+/*
+ * Latitude bands ("the sky map [can] be divided into latitude bands with minimal overlap ...
+ * convolution on the latitude bands is completely independent once the necessary overlap is included").
+ * A band is a range of BASE rings lo .. hi (1 <= lo <= hi <= 2 nside) together with the southern mirror
+ * rings 4 nside - hi .. 4 nside - lo, because the kernels evaluate a pair geometry once for both.
+ *
+ * sc_band_partition -- band `rank` of a split of the sphere into `world` bands of nearly equal pixel
+ * counts (1 <= world <= 2 nside).  HOST outputs, any may be NULL:
+ *   ring_lo, ring_hi   the band's base rings
+ *   out_rows[4]        pixel ranges [o0, o1) U [o2, o3) the band's convolution writes
+ *   in_rows[4]         pixel ranges [i0, i1) U [i2, i3) it reads (band + theta_max overlap); a range may be
+ *                      empty (x2 == x3) when the two parts merge at the equator
+ *
+ * sc_convolve_band -- sc_convolve restricted to one band: reads only in_rows of every input map, writes
+ * only out_rows of every output map (the other pixels are not touched).  Maps are full-size N_pix
+ * buffers as in sc_convolve, so rows exchanged between ranks land at their global positions.  The first
+ * call for a new band builds its tile list (synchronous); later calls are asynchronous on the stream.
+ */
+sc_status sc_band_partition(const sc_plan *plan, int world, int rank, int *ring_lo, int *ring_hi,
+                            int64_t *out_rows, int64_t *in_rows);
+sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float *const *in_maps,
+                           float *const *out_maps, int B, void *cuda_stream);
+
 /* Kernel launches enqueued by the last sc_convolve / sc_convolve_host on this plan. */
 int sc_last_launch_count(const sc_plan *plan);
 

@@ -14,6 +14,7 @@ SC_K_POLAR, SC_K_SYM, SC_K_BELT, SC_K_COUNT = 0, 1, 2, 3
 KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
 
 EXPORTS = ("sc_plan_create", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
+           "sc_band_partition", "sc_convolve_band",
            "sc_plan_destroy", "sc_plan_set_path",
            "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_last_launch_count",
            "sc_status_string", "sc_last_cuda_error", "sc_version")
@@ -44,6 +45,8 @@ def lib():
         l.sc_convolve_host.argtypes = [vp, vp, vp, i32]
         l.sc_convolve_profile.argtypes = [vp, vp, vp, i32, vp, vp]
         l.sc_plan_partition.argtypes = [vp, vp, vp]
+        l.sc_band_partition.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+        l.sc_convolve_band.argtypes = [vp, i32, i32, vp, vp, i32, vp]
         l.sc_plan_destroy.argtypes = [vp]
         l.sc_plan_set_path.argtypes = [vp, i32]
         l.sc_plan_info.argtypes = [vp, vp, vp, vp, vp]
@@ -109,6 +112,22 @@ def sc_plan_partition(plan):
     pr, fb = C.c_int(0), C.c_int(0)
     _chk(lib().sc_plan_partition(plan, C.byref(pr), C.byref(fb)), "sc_plan_partition")
     return dict(polar_rings=pr.value, first_belt_ring=fb.value)
+
+
+def sc_band_partition(plan, world, rank):
+    """-> dict(ring_lo, ring_hi, out_rows=(o0, o1, o2, o3), in_rows=(i0, i1, i2, i3)) of latitude band `rank`."""
+    lo, hi = C.c_int(0), C.c_int(0)
+    orow, irow = (C.c_int64 * 4)(), (C.c_int64 * 4)()
+    _chk(lib().sc_band_partition(plan, int(world), int(rank), C.byref(lo), C.byref(hi), orow, irow), "sc_band_partition")
+    return dict(ring_lo=lo.value, ring_hi=hi.value, out_rows=tuple(orow), in_rows=tuple(irow))
+
+
+def sc_convolve_band(plan, ring_lo, ring_hi, in_ptrs, out_ptrs, stream=0):
+    """sc_convolve restricted to base rings ring_lo .. ring_hi and their southern mirrors."""
+    if len(in_ptrs) != len(out_ptrs):
+        raise ValueError("in/out batch mismatch")
+    _chk(lib().sc_convolve_band(plan, int(ring_lo), int(ring_hi), _ptr_array(in_ptrs), _ptr_array(out_ptrs),
+                                len(in_ptrs), C.c_void_p(int(stream) or None)), "sc_convolve_band")
 
 
 def sc_plan_destroy(plan):
@@ -192,6 +211,16 @@ class Plan:
 
     def partition(self):
         return sc_plan_partition(self.handle)
+
+    def band(self, world, rank):
+        return sc_band_partition(self.handle, world, rank)
+
+    def convolve_band(self, ring_lo, ring_hi, maps, out):
+        """Band version of convolve(): reads/writes only the band's rows of the full-size tensors."""
+        import torch
+        sc_convolve_band(self.handle, ring_lo, ring_hi, [m.data_ptr() for m in maps], [o.data_ptr() for o in out],
+                         torch.cuda.current_stream().cuda_stream)
+        return out
 
     def convolve_host(self, maps, out=None):
         """maps: list of host fp32 numpy arrays or CPU tensors (N_pix) -> list of numpy arrays."""

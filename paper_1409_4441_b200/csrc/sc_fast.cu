@@ -23,6 +23,8 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <memory>
 #include <vector>
 
 namespace sc {
@@ -378,12 +380,92 @@ size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_
 cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
                         cudaStream_t st);
 
+// Host geometry kept for building tile lists after plan creation (latitude bands)
+struct HostGeo {
+    int N = 0, polar = 0;
+    std::vector<std::vector<PairEnt>> per_ring;   // per base ring 1 .. 2N: its input rings
+    std::vector<int> slot_of, pair_off;           // base ring -> slot; slot -> first entry of `pairs`
+    std::vector<char> is_belt;
+    int ipof(int r) const { return r < N ? r : (r <= 3 * N ? N : 4 * N - r); }
+    int shof(int r) const { return (r >= N && r <= 3 * N) ? ((r - N) & 1) : 0; }
+};
+
+// Sym-kernel tiles of the non-belt base rings r_lo .. r_hi, longest first, appended to `tiles`.  Tiles are
+// packed from runs of base pixels on one ring (32 R pixels per warp): whole runs of `run` pixels first, the
+// ragged remainders are bin-packed (first fit, decreasing); a tile holds at most W warps, kMaxSub runs and
+// Llimit staged positions (shared memory).  Returns the staged positions the tiles need.
+static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, int r_hi, int r_lo,
+                           std::vector<SymTile> &tiles) {
+    const int C = 32 * R;
+    struct SubH { int r, k0, n, nw; int Lcap; double work; };
+    auto make_sub = [&](int r, int k0, int n) {
+        SubH sb{r, k0, n, (n + C - 1) / C, 0, 0.0};
+        const int ip = g.ipof(r), sh = g.shof(r);
+        const int klast = k0 + n - 1;
+        for (const PairEnt &pe : g.per_ring[r]) {
+            const int w0 = ((2 * k0 + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) - pe.hw;
+            const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0;
+            sb.Lcap = std::max(sb.Lcap, L);
+            sb.work += (double)(2 * pe.hw + R);
+        }
+        sb.Lcap = (sb.Lcap + 7) & ~7;
+        sb.work *= sb.nw;
+        return sb;
+    };
+    std::vector<std::vector<SubH>> bins;
+    std::vector<SubH> partial;
+    for (int r = r_hi; r >= r_lo; --r) {
+        if (r <= g.polar || g.is_belt[r]) continue;
+        const int ip = g.ipof(r);
+        int k0 = 0;
+        for (; ip - k0 >= run; k0 += run) bins.push_back({make_sub(r, k0, run)});
+        if (k0 < ip) partial.push_back(make_sub(r, k0, ip - k0));
+    }
+    const size_t nfull = bins.size();
+    std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
+    std::vector<int> used(nfull, W), lsum(nfull, 0);
+    for (const SubH &sb : partial) {
+        size_t i = nfull;
+        for (; i < bins.size(); ++i)
+            if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Llimit) break;
+        if (i == bins.size()) { bins.emplace_back(); used.push_back(0); lsum.push_back(0); }
+        bins[i].push_back(sb); used[i] += sb.nw; lsum[i] += sb.Lcap;
+    }
+    std::vector<std::pair<double, size_t>> order;
+    int Lneed = 0;
+    for (size_t i = 0; i < bins.size(); ++i) {
+        double w = 0; int L = 0;
+        for (const SubH &sb : bins[i]) { w = std::max(w, sb.work / sb.nw); L += sb.Lcap; }
+        order.push_back({-w, i});
+        Lneed = std::max(Lneed, L);
+    }
+    std::stable_sort(order.begin(), order.end());
+    const size_t t0 = tiles.size();
+    tiles.resize(t0 + bins.size());
+    for (size_t t = 0; t < order.size(); ++t) {
+        const std::vector<SubH> &bn = bins[order[t].second];
+        SymTile &tl = tiles[t0 + t];
+        std::memset(&tl, 0, sizeof(tl));
+        tl.nsub = (int)bn.size();
+        int w0 = 0, soff = 0;
+        for (int i = 0; i < tl.nsub; ++i) {
+            const SubH &sb = bn[i];
+            const int slot = g.slot_of[sb.r];
+            tl.sub[i] = SubTile{sb.r, sb.k0, sb.n, g.pair_off[slot], g.pair_off[slot + 1] - g.pair_off[slot], w0, sb.nw, soff};
+            tl.nsteps = std::max(tl.nsteps, tl.sub[i].ne);
+            w0 += sb.nw; soff += sb.Lcap;
+        }
+    }
+    return Lneed;
+}
+
 struct FastCfg {            // per batch size
     bool ok = false;
     int threads = 0, R = 1, Ltot = 0;
     size_t smem = 0;
     SymTile *tiles = nullptr;     // [0, ntiles): all rings, work sorted; then the latitude chunks
-    int ntiles = 0, ntiles_all = 0;
+    int ntiles = 0, ntiles_all = 0, run = 0;
+    std::map<std::pair<int, int>, std::pair<SymTile *, int>> band_tiles;   // (ring lo, hi) -> device tile list
     std::vector<int> ch_off, ch_lo, ch_hi;   // chunk i: tiles [ch_off[i], ch_off[i+1]), base rings ch_lo[i] .. ch_hi[i]
 };
 
@@ -404,18 +486,40 @@ struct FastPlan {
     int *woff = nullptr;
     int4 *belt_tiles = nullptr;
     std::vector<int> bch_off, bch_lo, bch_hi;   // belt latitude chunks (tile offsets, base rings), equator first
+    std::shared_ptr<HostGeo> geo;
+    int belt_tiles_per_ring = 0;
 };
 
 template <int B, int R, int NC, bool TOT>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st,
-                              int t0, int nt) {
-    FastDev F{fp->pairs, c.tiles + t0, nt, fp->counter, c.Ltot, fp->ntab_s};
+                              const SymTile *tiles, int nt) {
+    FastDev F{fp->pairs, tiles, nt, fp->counter, c.Ltot, fp->ntab_s};
     cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, nt);
     if (grid <= 0) return cudaSuccess;
     sym_kernel<B, R, NC, TOT><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
+}
+
+// the sym kernel instance of this batch size over a tile list
+static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, int B, cudaStream_t st,
+                                const SymTile *tiles, int nt) {
+    cudaError_t e = cudaErrorInvalidValue;
+#define SC_SYM_CASE(BB, RR)                                                                  \
+    if (B == BB && c.R == RR)                                                                \
+        e = c.threads == 256 ? launch_sym<BB, RR, 256, true>(fp, c, P, io, st, tiles, nt)    \
+                             : launch_sym<BB, RR, 128, true>(fp, c, P, io, st, tiles, nt);
+    if (B == 1 && c.R == 4 && c.threads == 384) {
+        e = launch_sym<1, 4, 384, false>(fp, c, P, io, st, tiles, nt);
+    } else {
+        SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
+        SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
+        SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
+        SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
+    }
+#undef SC_SYM_CASE
+    return e;
 }
 
 // which: bit 0 = sym kernel, bit 1 = belt kernel (the two write disjoint pixels and may run on different
@@ -432,21 +536,7 @@ cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int w
             if (chunk + 1 >= (int)c.ch_off.size()) return cudaErrorInvalidValue;
             t0 = c.ch_off[chunk]; nt = c.ch_off[chunk + 1] - t0;
         }
-        e = cudaErrorInvalidValue;
-#define SC_SYM_CASE(BB, RR)                                                                  \
-    if (B == BB && c.R == RR)                                                                \
-        e = c.threads == 256 ? launch_sym<BB, RR, 256, true>(fp, c, P, io, st, t0, nt)       \
-                             : launch_sym<BB, RR, 128, true>(fp, c, P, io, st, t0, nt);
-        if (B == 1 && c.R == 4 && c.threads == 384) {
-            e = launch_sym<1, 4, 384, false>(fp, c, P, io, st, t0, nt);
-        } else {
-            SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
-            SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)
-            SC_SYM_CASE(3, 1) SC_SYM_CASE(3, 2)
-            SC_SYM_CASE(4, 1) SC_SYM_CASE(4, 2)
-        }
-#undef SC_SYM_CASE
-        if (e != cudaSuccess) return e;
+        if ((e = dispatch_sym(fp, c, P, io, B, st, c.tiles + t0, nt)) != cudaSuccess) return e;
         *launches += nt > 0 ? 1 : 0;
     }
     if ((which & 2) && fp->belt_ok) {
@@ -459,6 +549,43 @@ cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int w
             e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
             if (e == cudaSuccess) ++*launches;
         }
+    }
+    return e;
+}
+
+// Latitude band: the fast kernels over base rings lo .. hi only (1 <= lo <= hi <= 2N; their southern mirrors
+// included).  The sym tile list of a band is built on first use and cached (synchronous the first time).
+cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, int lo, int hi, cudaStream_t st,
+                             int *launches) {
+    *launches = 0;
+    if (!fp || B < 1 || B > kMaxB || !fp->cfg[B].ok) return cudaErrorInvalidValue;
+    FastCfg &c = fp->cfg[B];
+    const int N = P.nside;
+    cudaError_t e = cudaSuccess;
+    const int s_lo = std::max(lo, fp->polar + 1), s_hi = std::min(hi, std::min(fp->first_belt - 1, 2 * N));
+    if (s_lo <= s_hi) {
+        auto it = c.band_tiles.find({s_lo, s_hi});
+        if (it == c.band_tiles.end()) {
+            std::vector<SymTile> tiles;
+            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, tiles);
+            if (Lneed > c.Ltot) return cudaErrorInvalidValue;
+            SymTile *d = nullptr;
+            if ((e = cudaMalloc((void **)&d, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return e;
+            if (!tiles.empty() && (e = cudaMemcpy(d, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return e;
+            it = c.band_tiles.emplace(std::make_pair(s_lo, s_hi), std::make_pair(d, (int)tiles.size())).first;
+        }
+        if (it->second.second > 0) {
+            if ((e = dispatch_sym(fp, c, P, io, B, st, it->second.first, it->second.second)) != cudaSuccess) return e;
+            ++*launches;
+        }
+    }
+    const int b_lo = std::max(lo, fp->first_belt), b_hi = std::min(hi, 2 * N);
+    if (fp->belt_ok && b_lo <= b_hi) {
+        BeltDev F = fp->belt;                               // tile list: ring 2N first, belt_tiles_per_ring tiles per ring
+        F.tiles += (2 * N - b_hi) * fp->belt_tiles_per_ring;
+        F.ntiles = (b_hi - b_lo + 1) * fp->belt_tiles_per_ring;
+        e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
+        if (e == cudaSuccess) ++*launches;
     }
     return e;
 }
@@ -493,7 +620,10 @@ bool fast_available(const FastPlan *fp, int B) { return fp && B >= 1 && B <= kMa
 void fast_plan_destroy(FastPlan *fp) {
     if (!fp) return;
     cudaFree(fp->pairs); cudaFree(fp->pair_off); cudaFree(fp->counter);
-    for (auto &c : fp->cfg) cudaFree(c.tiles);
+    for (auto &c : fp->cfg) {
+        cudaFree(c.tiles);
+        for (auto &kv : c.band_tiles) cudaFree(kv.second.first);
+    }
     cudaFree(fp->woff); cudaFree(fp->belt_tiles);
     delete fp;
 }
@@ -579,6 +709,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     }
 
     FastPlan *fp = new FastPlan;
+    fp->geo = std::make_shared<HostGeo>();
     fp->ntab_s = ntab_s; fp->polar = polar; fp->nsm = nsm;
     auto fail = [&](cudaError_t e) { *err = e; fast_plan_destroy(fp); return (FastPlan *)nullptr; };
     cudaError_t e;
@@ -642,7 +773,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
             if ((e = cudaMemcpy(fp->belt_tiles, btiles.data(), btiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, (int)btiles.size(), pw_max, ne_max, nbuf, ntb};
-            fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true;
+            fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true; fp->belt_tiles_per_ring = N / T;
             // latitude chunks: the tile list runs from ring 2N down to the first belt ring, N / T tiles per ring
             {
                 int r_first = 2 * N + 1;
@@ -685,75 +816,15 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             cands.insert(cands.begin(), Cand{ft, fr});
         for (const Cand &cd : cands) {
             const int R = cd.R, W = cd.threads / 32, C = 32 * R;
-            struct SubH { int r, k0, n, nw; int Lcap; double work; };
-            auto make_sub = [&](int r, int k0, int n) {
-                SubH sb{r, k0, n, (n + C - 1) / C, 0, 0.0};
-                const int ip = ipof(r), sh = shof(r);
-                const int klast = k0 + n - 1;
-                for (const PairEnt &pe : per_ring[r]) {
-                    const int w0 = ((2 * k0 + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) - pe.hw;
-                    const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0;
-                    sb.Lcap = std::max(sb.Lcap, L);
-                    sb.work += (double)(2 * pe.hw + R);
-                }
-                sb.Lcap = (sb.Lcap + 7) & ~7;
-                sb.work *= sb.nw;
-                return sb;
-            };
             // full-width runs may be a little shorter than the CTA (last lanes idle) if that makes the
             // staged runs fit into shared memory
             for (int shrink = 0; shrink <= 64 && !c.ok; shrink += 16) {
             const int run = W * C - shrink;
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int Lmax = (int)(((size_t)smem_optin - 256 - tab_bytes) / ((size_t)2 * B * 2 * 16)) & ~7;
-            // tiles of the non-belt base rings r_lo .. r_hi, longest first; returns the staged positions needed
-            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tiles) -> int {
-                std::vector<std::vector<SubH>> bins;
-                std::vector<SubH> partial;
-                for (int r = r_hi; r >= r_lo; --r) {
-                    if (is_belt[r]) continue;
-                    const int ip = ipof(r);
-                    int k0 = 0;
-                    for (; ip - k0 >= run; k0 += run) bins.push_back({make_sub(r, k0, run)});
-                    if (k0 < ip) partial.push_back(make_sub(r, k0, ip - k0));
-                }
-                const size_t nfull = bins.size();
-                std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
-                std::vector<int> used(nfull, W), lsum(nfull, 0);
-                for (const SubH &sb : partial) {
-                    size_t i = nfull;
-                    for (; i < bins.size(); ++i)
-                        if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Lmax) break;
-                    if (i == bins.size()) { bins.emplace_back(); used.push_back(0); lsum.push_back(0); }
-                    bins[i].push_back(sb); used[i] += sb.nw; lsum[i] += sb.Lcap;
-                }
-                std::vector<std::pair<double, size_t>> order;
-                int Lneed = 0;
-                for (size_t i = 0; i < bins.size(); ++i) {
-                    double w = 0; int L = 0;
-                    for (const SubH &sb : bins[i]) { w = std::max(w, sb.work / sb.nw); L += sb.Lcap; }
-                    order.push_back({-w, i});
-                    Lneed = std::max(Lneed, L);
-                }
-                std::stable_sort(order.begin(), order.end());
-                const size_t t0 = tiles.size();
-                tiles.resize(t0 + bins.size());
-                for (size_t t = 0; t < order.size(); ++t) {
-                    const std::vector<SubH> &bn = bins[order[t].second];
-                    SymTile &tl = tiles[t0 + t];
-                    std::memset(&tl, 0, sizeof(tl));
-                    tl.nsub = (int)bn.size();
-                    int w0 = 0, soff = 0;
-                    for (int i = 0; i < tl.nsub; ++i) {
-                        const SubH &sb = bn[i];
-                        const int slot = slot_of[sb.r];
-                        tl.sub[i] = SubTile{sb.r, sb.k0, sb.n, pair_off[slot], pair_off[slot + 1] - pair_off[slot], w0, sb.nw, soff};
-                        tl.nsteps = std::max(tl.nsteps, tl.sub[i].ne);
-                        w0 += sb.nw; soff += sb.Lcap;
-                    }
-                }
-                return Lneed;
-            };
+            HostGeo &g = *fp->geo;
+            g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, tl); };
             // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
             // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
             std::vector<SymTile> tiles;
@@ -778,7 +849,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const size_t smem = tab_bytes + (size_t)2 * B * 2 * Ltot * 16;
             if (smem + 256 > (size_t)smem_optin) continue;        // 256: static shared memory (barriers)
             c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
-            c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all;
+            c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all; c.run = run;
             if ((e = cudaMalloc((void **)&c.tiles, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return fail(e);
             if (!tiles.empty() && (e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             c.ok = true;

@@ -24,6 +24,7 @@ cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cud
 int fast_first_belt_ring(const FastPlan *fp);
 cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches, int chunk);
 int fast_chunk_count(const FastPlan *fp, int B, int kind);
+cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, int lo, int hi, cudaStream_t st, int *launches);
 void fast_chunk_rings(const FastPlan *fp, int B, int kind, int i, int *lo, int *hi);
 bool fast_available(const FastPlan *fp, int B);
 }  // namespace sc
@@ -92,7 +93,7 @@ struct sc_plan {
     int stage_maps = 0;
     cudaStream_t own_stream = nullptr, comp_stream = nullptr, d2h_stream = nullptr;
     std::vector<cudaEvent_t> events;           // pool for the pipelined host entry
-    std::vector<int> rlo_h;                    // host copy of the first candidate input ring of every ring
+    std::vector<int> rlo_h, rhi_h;             // host copies of the candidate input-ring interval of every ring
     mutable int last_launches = 0;
     sc::FastPlan *fast = nullptr;
     int polar_rings = 0;                       // rings 1..polar_rings and their southern mirrors use the generic kernel
@@ -262,7 +263,7 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
             if (hi < nr) ++hi;
             rlo[i - 1] = lo; rhi[i - 1] = hi;
         }
-        pl->rlo_h = rlo;
+        pl->rlo_h = rlo; pl->rhi_h = rhi;
         // device table in the reversed coordinate t = (1 - x) (n-1)/(1-c): node j of the device
         // table is caller node n-1-j.  Cell [j, j+1): K = a_j + t b_j with b_j = T'_{j+1} - T'_j,
         // a_j = T'_j - j b_j  (fp64, rounded once).  Zero padding after the last cell.
@@ -526,6 +527,88 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
     }
     plan->last_launches = launches;
     SC_CUDA(cudaStreamSynchronize(s_out));
+    return SC_OK;
+}
+
+static void band_rows(const sc_plan *plan, int lo, int hi, int64_t *out_rows, int64_t *in_rows) {
+    const int N = plan->dev.nside, N4 = 4 * N;
+    const int64_t npix = plan->dev.npix;
+    auto row = [&](int ring) -> int64_t { return ring <= N4 - 1 ? (int64_t)plan->rings[ring - 1].start : npix; };
+    if (out_rows) {
+        out_rows[0] = row(lo); out_rows[1] = row(hi + 1);
+        out_rows[2] = hi >= 2 * N ? row(2 * N + 1) : row(N4 - hi); out_rows[3] = row(N4 - lo + 1);
+    }
+    if (in_rows) {
+        const int a = std::max(1, plan->rlo_h[lo - 1] - 1), b = std::min(N4 - 1, plan->rhi_h[hi - 1] + 1);
+        in_rows[0] = row(a); in_rows[1] = row(b + 1);
+        in_rows[2] = row(N4 - b); in_rows[3] = row(N4 - a + 1);
+        if (in_rows[2] <= in_rows[1]) { in_rows[1] = in_rows[3]; in_rows[2] = in_rows[3]; }   // merged at the equator
+    }
+}
+
+sc_status sc_band_partition(const sc_plan *plan, int world, int rank, int *ring_lo, int *ring_hi,
+                            int64_t *out_rows, int64_t *in_rows) {
+    if (!plan) return SC_ERR_INVALID_ARG;
+    const int N = plan->dev.nside;
+    if (world < 1 || world > 2 * N || rank < 0 || rank >= world) return SC_ERR_INVALID_ARG;
+    // base ring r stands for rings r and 4N - r: 2 n_r pixels (n_r for the equator ring 2N)
+    const int64_t total = plan->dev.npix;
+    auto first_ring = [&](int k) -> int {            // first base ring of band k (band `world` starts at 2N + 1)
+        if (k <= 0) return 1;
+        if (k >= world) return 2 * N + 1;
+        int64_t cum = 0;
+        int r = 1;
+        for (; r <= 2 * N; ++r) {
+            if (cum * world >= total * k) break;
+            cum += (int64_t)plan->rings[r - 1].n * (r < 2 * N ? 2 : 1);
+        }
+        // every band keeps at least one ring
+        return std::min(std::max(r, k + 1), 2 * N - (world - 1 - k));
+    };
+    const int lo = first_ring(rank), hi = first_ring(rank + 1) - 1;
+    if (hi < lo) return SC_ERR_INVALID_ARG;
+    if (ring_lo) *ring_lo = lo;
+    if (ring_hi) *ring_hi = hi;
+    band_rows(plan, lo, hi, out_rows, in_rows);
+    return SC_OK;
+}
+
+sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float *const *in_maps,
+                           float *const *out_maps, int B, void *cuda_stream) {
+    if (!plan || !in_maps || !out_maps || B < 1) return SC_ERR_INVALID_ARG;
+    const sc::Dev &D = plan->dev;
+    const int N = D.nside;
+    if (ring_lo < 1 || ring_hi < ring_lo || ring_hi > 2 * N) return SC_ERR_INVALID_ARG;
+    for (int b = 0; b < B; ++b) {
+        if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
+        if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return SC_ERR_INVALID_ARG;
+        for (int a = 0; a < B; ++a) if ((const float *)out_maps[b] == in_maps[a]) return SC_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int64_t orow[4];
+    band_rows(plan, ring_lo, ring_hi, orow, nullptr);
+    int launches = 0;
+    for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
+        const int nb = std::min(sc::kMaxB, B - b0);
+        sc::Maps io{};
+        for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
+        if (plan->path == SC_PATH_GENERIC || !sc::fast_available(plan->fast, nb)) {
+            SC_CUDA(sc::launch_generic_conv(D, io, nb, (int)orow[0], (int)orow[1], (int)orow[2], (int)orow[3], st));
+            ++launches;
+            continue;
+        }
+        const int pr = plan->polar_rings;
+        if (ring_lo <= pr) {                               // rings next to the poles
+            int64_t prow[4];
+            band_rows(plan, ring_lo, std::min(ring_hi, pr), prow, nullptr);
+            SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, (int)prow[0], (int)prow[1], (int)prow[2], (int)prow[3], st));
+            ++launches;
+        }
+        int nl = 0;
+        SC_CUDA(sc::fast_launch_band(plan->fast, D, io, nb, ring_lo, ring_hi, st, &nl));
+        launches += nl;
+    }
+    plan->last_launches = launches;
     return SC_OK;
 }
 
