@@ -55,3 +55,102 @@ def gather_outputs(local_out, n_maps, group=None):
         for i, o in zip(map_shard(n_maps, r, world), parts[r]):
             out[i] = o
     return out
+
+
+# ---------------------------------------------------------------------------------------------------
+# One map over several ranks: latitude bands with overlap.  Rank r owns the input and
+# output rows `out_rows` of band r (sc_band_partition); before the convolution it needs the overlap
+# rows in_rows - out_rows from the ranks that own them (halo exchange, point to point), afterwards
+# the bands are independent.  Maps are full-size N_pix tensors on every rank so that rows land at
+# their global positions; only the band's rows are ever valid / touched.
+# ---------------------------------------------------------------------------------------------------
+
+def _ranges(rows):
+    """(a, b, c, d) -> list of non-empty half-open pixel ranges."""
+    a, b, c, d = (int(x) for x in rows)
+    return [(lo, hi) for lo, hi in ((a, b), (c, d)) if hi > lo]
+
+
+def _intersect(xs, ys):
+    out = []
+    for a, b in xs:
+        for c, d in ys:
+            lo, hi = max(a, c), min(b, d)
+            if hi > lo:
+                out.append((lo, hi))
+    return sorted(out)
+
+
+def _subtract(xs, ys):
+    out = []
+    for a, b in xs:
+        cur = [(a, b)]
+        for c, d in ys:
+            nxt = []
+            for lo, hi in cur:
+                if d <= lo or c >= hi:
+                    nxt.append((lo, hi))
+                else:
+                    if c > lo:
+                        nxt.append((lo, c))
+                    if d < hi:
+                        nxt.append((d, hi))
+            cur = nxt
+        out += cur
+    return sorted(out)
+
+
+def halo_plan(bands, rank):
+    """bands: per rank dict(out_rows=(..4), in_rows=(..4)).  -> (sends, recvs): lists of (peer, lo, hi)
+    pixel ranges this rank must send to / receive from each peer, in a deterministic order."""
+    own = [_ranges(b["out_rows"]) for b in bands]
+    need = [_subtract(_ranges(b["in_rows"]), own[r]) for r, b in enumerate(bands)]
+    sends, recvs = [], []
+    for peer in range(len(bands)):
+        if peer == rank:
+            continue
+        sends += [(peer, lo, hi) for lo, hi in _intersect(need[peer], own[rank])]
+        recvs += [(peer, lo, hi) for lo, hi in _intersect(need[rank], own[peer])]
+    return sends, recvs
+
+
+def exchange_halos(maps, bands, rank, group=None):
+    """Fill the overlap rows of the full-size tensors `maps` (valid in this rank's out_rows) from their
+    owners.  Point-to-point, one message per (peer, range, map); bytes = the overlap only."""
+    import torch.distributed as dist
+    sends, recvs = halo_plan(bands, rank)
+    ops, keep = [], []
+    for m in maps:
+        for peer, lo, hi in recvs:
+            ops.append(dist.P2POp(dist.irecv, m[lo:hi], peer, group))
+        for peer, lo, hi in sends:
+            buf = m[lo:hi].contiguous()
+            keep.append(buf)
+            ops.append(dist.P2POp(dist.isend, buf, peer, group))
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+    return sum(hi - lo for _, lo, hi in recvs) * len(maps)
+
+
+def gather_bands(maps, bands, group=None):
+    """Make every rank's full-size tensors complete: each band's rows are broadcast by their owner."""
+    import torch.distributed as dist
+    for m in maps:
+        for owner, b in enumerate(bands):
+            for lo, hi in _ranges(b["out_rows"]):
+                dist.broadcast(m[lo:hi], src=owner, group=group)
+
+
+def convolve_banded(plan, maps_in, maps_out, group=None, gather=False):
+    """Convolve maps sharded by latitude bands over the ranks of `group` with `plan` (a Plan built on
+    every rank): halo exchange, then the rank's band through sc_convolve_band.  maps_in: full-size CUDA
+    tensors valid in this rank's band rows; maps_out: full-size CUDA tensors, band rows written."""
+    import torch.distributed as dist
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    bands = [plan.band(world, r) for r in range(world)]
+    exchange_halos(maps_in, bands, rank, group)
+    plan.convolve_band(bands[rank]["ring_lo"], bands[rank]["ring_hi"], maps_in, maps_out)
+    if gather:
+        gather_bands(maps_out, bands, group)
+    return bands[rank]
