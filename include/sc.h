@@ -86,8 +86,10 @@ sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *c
 
 /*
  * sc_convolve_host -- the same operation with HOST buffers (the end-to-end call): copies the B
- * input maps to plan-owned device staging buffers, runs sc_convolve, copies the results back and
- * synchronises.  in/out: HOST arrays of B HOST pointers to N_pix fp32 each (pinned memory makes
+ * input maps to plan-owned device staging buffers, runs the kernels of sc_convolve, copies the results
+ * back and synchronises.  On the AUTO path the three steps are pipelined over latitude chunks on three
+ * streams (a chunk is computed as soon as its rows have arrived and returned while later chunks are
+ * still in flight); the results are identical to sc_convolve's.  in/out: HOST arrays of B HOST pointers to N_pix fp32 each (pinned memory makes
  * the copies faster but is not required).
  */
 sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host,
@@ -182,7 +184,7 @@ int sc_last_launch_count(const sc_plan *plan);
 const char *sc_status_string(sc_status s);
 /* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
 const char *sc_last_cuda_error(void);
-/* Library version, e.g. "sc 0.1 (sm_100a)". */
+/* Library version, e.g. "sc 0.2 (sm_100a)". */
 const char *sc_version(void);
 
 #ifdef __cplusplus

@@ -471,7 +471,6 @@ struct FastCfg {            // per batch size
 
 struct FastPlan {
     PairEnt *pairs = nullptr;
-    int *counter = nullptr;
     int ntab_s = 0;
     int polar = 0;
     int first_belt = 0;           // base rings first_belt .. 2N go to the belt kernel (2N + 1: none)
@@ -493,7 +492,7 @@ struct FastPlan {
 template <int B, int R, int NC, bool TOT>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st,
                               const SymTile *tiles, int nt) {
-    FastDev F{fp->pairs, tiles, nt, fp->counter, c.Ltot, fp->ntab_s};
+    FastDev F{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s};
     cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, nt);
@@ -619,7 +618,7 @@ bool fast_available(const FastPlan *fp, int B) { return fp && B >= 1 && B <= kMa
 
 void fast_plan_destroy(FastPlan *fp) {
     if (!fp) return;
-    cudaFree(fp->pairs); cudaFree(fp->pair_off); cudaFree(fp->counter);
+    cudaFree(fp->pairs); cudaFree(fp->pair_off);
     for (auto &c : fp->cfg) {
         cudaFree(c.tiles);
         for (auto &kv : c.band_tiles) cudaFree(kv.second.first);
@@ -715,7 +714,6 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     cudaError_t e;
     if ((e = cudaMalloc((void **)&fp->pairs, std::max<size_t>(pairs.size(), 1) * sizeof(PairEnt))) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc((void **)&fp->pair_off, pair_off.size() * sizeof(int))) != cudaSuccess) return fail(e);
-    if ((e = cudaMalloc((void **)&fp->counter, sizeof(int))) != cudaSuccess) return fail(e);
     if ((e = cudaMemcpy(fp->pairs, pairs.data(), pairs.size() * sizeof(PairEnt), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
     if ((e = cudaMemcpy(fp->pair_off, pair_off.data(), pair_off.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
 
@@ -818,7 +816,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int R = cd.R, W = cd.threads / 32, C = 32 * R;
             // full-width runs may be a little shorter than the CTA (last lanes idle) if that makes the
             // staged runs fit into shared memory
-            for (int shrink = 0; shrink <= 64 && !c.ok; shrink += 16) {
+            for (int shrink = 0; shrink <= W * C / 4 && !c.ok; shrink += 16) {
             const int run = W * C - shrink;
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int Lmax = (int)(((size_t)smem_optin - 256 - tab_bytes) / ((size_t)2 * B * 2 * 16)) & ~7;

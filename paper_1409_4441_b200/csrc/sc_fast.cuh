@@ -36,7 +36,6 @@ struct FastDev {
     const PairEnt *pairs;
     const SymTile *tiles;
     int ntiles;
-    int *counter;
     int Ltot;               // staged positions per plane
     int ntab_s;             // entries of the shared-memory table
 };

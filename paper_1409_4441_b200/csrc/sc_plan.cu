@@ -205,7 +205,7 @@ const char *sc_status_string(sc_status s) {
 }
 
 const char *sc_last_cuda_error(void) { return g_cuda_err.c_str(); }
-const char *sc_version(void) { return "sc 0.1 (sm_100a)"; }
+const char *sc_version(void) { return "sc 0.2 (sm_100a)"; }
 
 sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *ktable, int n_table,
                          double theta_max, int max_batch) {
