@@ -149,6 +149,27 @@ def test_config5_sampled_batch3(sc):
     _sampled_config(sc, 5, (2048, 60), 4000, 50000)
 
 
+def test_config6_paper_scale_sampled(sc):
+    """The paper's own operating point (theta_cut 240', ~61,000 neighbours per pixel): counts
+    and values on 300 sampled pixels.  The belt tap arrays do not fit at this disc size, so the sym kernel
+    (two accumulator sets) covers the belt as well."""
+    cfg = gen.config(6)
+    T, maps = gen.table_for(cfg), gen.maps_for(cfg)
+    sel = gen.sample_pixels(cfg.nside, 300, seed=66)
+    ref, cnt, sig = O.convolve(cfg.nside, T, cfg.theta_max, maps, sel=sel)
+    with sc.Plan(cfg.nside, T, cfg.theta_max, 1) as plan:
+        info = plan.info()
+        assert info["max_t_err"] < info["guard_band"]
+        c, s = plan.neighbour_counts()
+        c, s = c.cpu().numpy(), s.cpu().numpy().view(np.uint64)
+        assert int(c.astype(np.int64).sum()) == info["total_pairs"]
+        np.testing.assert_array_equal(c[sel], cnt)
+        np.testing.assert_array_equal(s[sel], sig)
+        out = _gpu_convolve(sc, plan, maps)
+        _check_values(out[0][sel], ref[0], "cfg6 paper scale")
+        assert np.all(np.isfinite(out[0]))
+
+
 @pytest.mark.parametrize("path", PATHS)
 def test_paths_agree_config3_rings(sc, path):
     """Whole rings at Nside 1024 (several tiles + ragged tails): pole rings, a mid-cap ring, the

@@ -47,11 +47,15 @@ CONFIGS = (
     Config("cfg4_nside2048_split5am", 2048, 20 * ARCMIN, 16384, "split", 5 * ARCMIN, (3,),
            extra=dict(l_split=1500, taper_from=15 * ARCMIN)),
     Config("cfg5_nside2048_gauss20am_b3", 2048, 60 * ARCMIN, 16384, "gauss", 20 * ARCMIN, (4, 5, 6)),
+    # NOT a BASELINE.json config: the paper's own worked example (7' beam, l_cut 1500, theta_cut 240',
+    # PAPER.md:94-96, Fig. 3-4) as a split-like stand-in table -- context for Eq. 7's 8.0 s on a GTX 480
+    Config("cfg6_paper_nside2048_split7am_240am", 2048, 240 * ARCMIN, 16384, "split", 7 * ARCMIN, (7,),
+           extra=dict(l_split=1500, taper_from=200 * ARCMIN)),
 )
 
 
 def config(i: int) -> Config:
-    """BASELINE.json configs[i-1] (1-based as in SURVEY.md)."""
+    """BASELINE.json configs[i-1] (1-based as in SURVEY.md); 6 = the paper-scale extra (see CONFIGS)."""
     return CONFIGS[i - 1]
 
 
