@@ -154,21 +154,25 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 const int r = tl.x, k0 = tl.y, ne = tl.w;
                 const int sh = (r - N) & 1;
                 const int e0 = F.pair_off[tl.z];
+                const int g0 = F.grp_off[tl.z], ngrp = F.grp_off[tl.z + 1] - g0 - 1;
+                for (int b = 0; b < B; ++b)                                  // the consumers walk the groups once per map
+                for (int gi = 0; gi < ngrp; ++gi) {
                 unsigned char *tbuf = tapbase + (size_t)tb * TL.bytes;
                 float2 *S = reinterpret_cast<float2 *>(tbuf);
                 int4 *desc = reinterpret_cast<int4 *>(tbuf + TL.desc);
                 int *exc_e = reinterpret_cast<int *>(tbuf + TL.exc_e), *exc_j = reinterpret_cast<int *>(tbuf + TL.exc_j);
                 float *exc_k = reinterpret_cast<float *>(tbuf + TL.exc_k);
                 int *nexc = reinterpret_cast<int *>(tbuf + TL.nexc);
+                const int ge0 = F.grp_e[g0 + gi], ge1 = F.grp_e[g0 + gi + 1];    // input rings of this group
                 mbar_wait_sleep(&tap_empty[tb], tpar ^ 1u);                   // consumers are done with this buffer
                 if (pt == 0) *nexc = 0;
                 bar_named(1, kTapThreads);
-                for (int e = 0; e < ne; ++e) {
+                for (int e = ge0; e < ge1; ++e) {
                     const PairEnt pe = F.pairs[e0 + e];
                     const int wo = F.woff[e0 + e];
                     int delta, w0a, a0, ng;
                     belt_window(pe, sh, k0, delta, w0a, a0, ng);
-                    if (pt == 0) desc[e] = make_int4(ng, wo * 8, 2 * pe.hw + 1, 0);
+                    if (pt == 0) desc[e - ge0] = make_int4(ng, wo * 8, 2 * pe.hw + 1, 0);
                     // nearest pixel of ring rq in azimuth: kc = k + delta, at angle dcc from p.  In the belt
                     // Y = N (2k + 1 - sh + shq), so delta = (1 - sh + shq) >> 1 and the remainder is N or 0.
                     const int Yk = 1 - sh + pe.shq;
@@ -197,6 +201,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 }
                 mbar_arrive(&tap_full[tb]);
                 if (++tb == NTB) { tb = 0; tpar ^= 1u; }
+                }
             }
         }
         return;
@@ -211,13 +216,10 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
         const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
         if (tile >= F.ntiles) continue;
         const int4 tl = F.tiles[tile];
-        const int r = tl.x, k0 = tl.y, ne = tl.w;
+        const int r = tl.x, k0 = tl.y;
         const int sh = (r - N) & 1;
         const int e0 = F.pair_off[tl.z];
-        const unsigned char *tbuf = tapbase + (size_t)tb * TL.bytes;
-        const int4 *desc = reinterpret_cast<const int4 *>(tbuf + TL.desc);
-        mbar_wait(&tap_full[tb], tpar);                       // taps of this tile are in place
-        const int nexc = *reinterpret_cast<const int *>(tbuf + TL.nexc);
+        const int g0 = F.grp_off[tl.z], ngrp = F.grp_off[tl.z + 1] - g0 - 1;   // groups of input rings whose taps fit a buffer
 
         for (int b = 0; b < B; ++b) {
             const float *__restrict__ in = io.in[b];
@@ -228,8 +230,14 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
             }
             int ntaps = 0;
-            for (int e = 0; e < ne; ++e) {
-                const int4 d = desc[e];                                   // (chunks, tap offset in bytes, taps)
+            for (int gi = 0; gi < ngrp; ++gi) {
+            const unsigned char *tbuf = tapbase + (size_t)tb * TL.bytes;
+            const int4 *desc = reinterpret_cast<const int4 *>(tbuf + TL.desc);
+            const int ge0 = F.grp_e[g0 + gi], ge1 = F.grp_e[g0 + gi + 1];
+            mbar_wait(&tap_full[tb], tpar);                       // taps of this group are in place
+            const int nexc = *reinterpret_cast<const int *>(tbuf + TL.nexc);
+            for (int e = ge0; e < ge1; ++e) {
+                const int4 d = desc[e - ge0];                             // (chunks, tap offset in bytes, taps)
                 const float4 *S4 = reinterpret_cast<const float4 *>(tbuf + d.y);   // S4[2 g + i] = S[4 g + 2 i .. + 1]
                 const float *pl = stage + (size_t)buf * 8 * LP + 4 * tid;
                 mbar_wait(&full_bar[buf], par);
@@ -280,7 +288,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
                 if (++buf == NBUF) { buf = 0; par ^= 1u; }
                 ntaps += d.z;
-                if (TOT && (ntaps >= 48 || e + 1 == ne)) {
+                if (TOT && (ntaps >= 48 || e + 1 == ge1)) {
 #pragma unroll
                     for (int g = 0; g < 8; ++g) {
                         tot01[g] = __fadd2_rn(tot01[g], acc01[g]); tot23[g] = __fadd2_rn(tot23[g], acc23[g]);
@@ -290,15 +298,12 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 }
             }
 
-            if (!TOT) {
-#pragma unroll
-                for (int g = 0; g < 8; ++g) { tot01[g] = acc01[g]; tot23[g] = acc23[g]; }
-            }
-            // ---- uncertain taps: canonical fp64 decision per pixel pair and image ------------------
+            // ---- uncertain taps of this group: canonical fp64 decision per pixel pair and image -----
             if (nexc > 0) {
+                float2 *s01 = TOT ? tot01 : acc01, *s23 = TOT ? tot23 : acc23;     // the set that holds the sums so far
                 float tt[4][8];
 #pragma unroll
-                for (int g = 0; g < 8; ++g) { tt[0][g] = tot01[g].x; tt[1][g] = tot01[g].y; tt[2][g] = tot23[g].x; tt[3][g] = tot23[g].y; }
+                for (int g = 0; g < 8; ++g) { tt[0][g] = s01[g].x; tt[1][g] = s01[g].y; tt[2][g] = s23[g].x; tt[3][g] = s23[g].y; }
                 auto apply = [&](const PairEnt &pe, int j, float Ku) {
                     const int delta = (1 - sh + pe.shq) >> 1;
 #pragma unroll
@@ -321,7 +326,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     const float *exc_k = reinterpret_cast<const float *>(tbuf + TL.exc_k);
                     for (int i = 0; i < nexc; ++i) apply(F.pairs[e0 + exc_e[i]], exc_j[i], exc_k[i]);
                 } else {                              // list overflow: rescan every tap (never seen in practice)
-                    for (int e = 0; e < ne; ++e) {
+                    for (int e = ge0; e < ge1; ++e) {
                         const PairEnt pe = F.pairs[e0 + e];
                         const int Yk = 1 - sh + pe.shq;
                         const float dcc = (float)(N - ((Yk & 1) ? N : 0)) * pe.cdc;
@@ -333,7 +338,15 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     }
                 }
 #pragma unroll
-                for (int g = 0; g < 8; ++g) { tot01[g] = make_float2(tt[0][g], tt[1][g]); tot23[g] = make_float2(tt[2][g], tt[3][g]); }
+                for (int g = 0; g < 8; ++g) { s01[g] = make_float2(tt[0][g], tt[1][g]); s23[g] = make_float2(tt[2][g], tt[3][g]); }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&tap_empty[tb]);                   // tap buffer may be refilled
+            if (++tb == NTB) { tb = 0; tpar ^= 1u; }
+            }
+            if (!TOT) {
+#pragma unroll
+                for (int g = 0; g < 8; ++g) { tot01[g] = acc01[g]; tot23[g] = acc23[g]; }
             }
 
             // ---- store: 4 consecutive pixels per image -> one 16-byte store ------------------------
@@ -348,9 +361,6 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 *reinterpret_cast<float4 *>(out + ((g < 4) ? start_n : start_s) + k + (g & 3) * N) = v;
             }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&tap_empty[tb]);                       // tap buffer may be refilled
-        if (++tb == NTB) { tb = 0; tpar ^= 1u; }
     }
 }
 
@@ -369,12 +379,13 @@ static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io
 }
 
 // variants: (512 consumer threads, slack 64, single accumulator set) for small discs on Nside % 2048 == 0;
-// (256 | 128, slack 256, two accumulator sets) otherwise
-cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
+// (256 | 128, slack 256 or 512, two accumulator sets) otherwise
+cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, size_t smem, int nsm,
                         cudaStream_t st) {
-    if (threads == 512) return launch_belt_nc<512, 64, false>(P, F, io, B, smem, nsm, st);
-    if (threads == 256) return launch_belt_nc<256, 256, true>(P, F, io, B, smem, nsm, st);
-    if (threads == 128) return launch_belt_nc<128, 256, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 512 && slack == 64) return launch_belt_nc<512, 64, false>(P, F, io, B, smem, nsm, st);
+    if (threads == 256 && slack == 256) return launch_belt_nc<256, 256, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 256 && slack == 512) return launch_belt_nc<256, 512, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 128 && slack == 256) return launch_belt_nc<128, 256, true>(P, F, io, B, smem, nsm, st);
     return cudaErrorInvalidValue;
 }
 

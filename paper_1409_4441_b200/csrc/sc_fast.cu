@@ -377,7 +377,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 // host side
 // ---------------------------------------------------------------------------------------------
 size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_max);
-cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, size_t smem, int nsm,
+cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, size_t smem, int nsm,
                         cudaStream_t st);
 
 // Host geometry kept for building tile lists after plan creation (latitude bands)
@@ -486,7 +486,8 @@ struct FastPlan {
     int4 *belt_tiles = nullptr;
     std::vector<int> bch_off, bch_lo, bch_hi;   // belt latitude chunks (tile offsets, base rings), equator first
     std::shared_ptr<HostGeo> geo;
-    int belt_tiles_per_ring = 0;
+    int belt_tiles_per_ring = 0, belt_slack = 0;
+    int *grp_off = nullptr, *grp_e = nullptr;
 };
 
 template <int B, int R, int NC, bool TOT>
@@ -545,7 +546,7 @@ cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int w
             F.tiles += fp->bch_off[chunk]; F.ntiles = fp->bch_off[chunk + 1] - fp->bch_off[chunk];
         }
         if (F.ntiles > 0) {
-            e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
+            e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_slack, fp->belt_smem, fp->nsm, st);
             if (e == cudaSuccess) ++*launches;
         }
     }
@@ -583,7 +584,7 @@ cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, 
         BeltDev F = fp->belt;                               // tile list: ring 2N first, belt_tiles_per_ring tiles per ring
         F.tiles += (2 * N - b_hi) * fp->belt_tiles_per_ring;
         F.ntiles = (b_hi - b_lo + 1) * fp->belt_tiles_per_ring;
-        e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_smem, fp->nsm, st);
+        e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_slack, fp->belt_smem, fp->nsm, st);
         if (e == cudaSuccess) ++*launches;
     }
     return e;
@@ -623,7 +624,7 @@ void fast_plan_destroy(FastPlan *fp) {
         cudaFree(c.tiles);
         for (auto &kv : c.band_tiles) cudaFree(kv.second.first);
     }
-    cudaFree(fp->woff); cudaFree(fp->belt_tiles);
+    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->grp_off); cudaFree(fp->grp_e);
     delete fp;
 }
 
@@ -726,7 +727,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     {
         const double mean_nb_b = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
         if (N % 2048 == 0 && mean_nb_b <= 1000.0 && !std::getenv("SC_BELT_NO512")) bvars.push_back({512, 64});
-        if (N % 1024 == 0) bvars.push_back({256, 256});
+        if (N % 1024 == 0) { bvars.push_back({256, 256}); bvars.push_back({256, 512}); }
         else if (N % 512 == 0) bvars.push_back({128, 256});
     }
     for (const BeltVar &bv : bvars) {
@@ -737,23 +738,34 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         std::vector<int4> btiles;
         int pw_max = 0, ne_max = 0;
         bool fits = true;
+        // The input rings of a base ring are cut into groups whose tap arrays fit one tap buffer (a few
+        // hundred rings of a few hundred taps for paper-scale discs do not fit as a whole).
+        const int kTapCap = 2048, kGroupRings = 96;                       // float2 entries, rings per group
+        std::vector<int> grp_off(1, 0), grp_e;
         std::fill(is_belt.begin(), is_belt.end(), 0);
-        for (int r = 2 * N; r > polar; --r) {
-            if (ipof(r) != N) continue;
-            bool all = true;
+        for (int r = polar + 1; r <= 2 * N; ++r) {                           // slots run over base rings polar+1 .. 2N
+            bool all = ipof(r) == N;
             for (const PairEnt &pe : per_ring[r]) if (pe.ipq != N) { all = false; break; }
-            if (!all) continue;
-            is_belt[r] = 1;
-            int off = 0;
+            is_belt[r] = all;
             const int base = pair_off[slot_of[r]];
+            int off = 0, cnt = 0;
+            grp_e.push_back(0);
             for (size_t i = 0; i < per_ring[r].size(); ++i) {
                 const int ng_max = (2 * per_ring[r][i].hw + 4 + 3 + 3) >> 2;   // chunks of 4 staged positions
-                if (4 * ng_max > bv.slack + 4) fits = false;                    // plane = T - 4 + 4 ng floats
+                const int len = (4 * ng_max + 2 + 1) & ~1;                     // tap pairs, even count
+                if (all && (4 * ng_max > bv.slack + 4 || len > kTapCap)) fits = false;   // plane = T - 4 + 4 ng floats
+                if (cnt > 0 && (off + len > kTapCap || cnt >= kGroupRings)) {  // next group
+                    grp_e.push_back((int)i); off = 0; cnt = 0;
+                }
                 woff[base + i] = off;
-                off += (4 * ng_max + 2 + 1) & ~1;                              // tap pairs, even count
+                off += len; ++cnt;
+                if (all) { pw_max = std::max(pw_max, off); ne_max = std::max(ne_max, cnt); }
             }
-            pw_max = std::max(pw_max, off);
-            ne_max = std::max(ne_max, (int)per_ring[r].size());
+            grp_e.push_back((int)per_ring[r].size());
+            grp_off.push_back((int)grp_e.size());
+        }
+        for (int r = 2 * N; r > polar; --r) {
+            if (!is_belt[r]) { for (int q = r; q > polar; --q) is_belt[q] = 0; break; }   // belt rings are contiguous from 2N down
             for (int k0 = 0; k0 < N; k0 += T) btiles.push_back(make_int4(r, k0, slot_of[r], (int)per_ring[r].size()));
         }
         int nbuf = 0, ntb = 0;
@@ -770,7 +782,12 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((e = cudaMemcpy(fp->woff, woff.data(), woff.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
             if ((e = cudaMemcpy(fp->belt_tiles, btiles.data(), btiles.size() * sizeof(int4), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
-            fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, (int)btiles.size(), pw_max, ne_max, nbuf, ntb};
+            if ((e = cudaMalloc((void **)&fp->grp_off, grp_off.size() * sizeof(int))) != cudaSuccess) return fail(e);
+            if ((e = cudaMemcpy(fp->grp_off, grp_off.data(), grp_off.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+            if ((e = cudaMalloc((void **)&fp->grp_e, grp_e.size() * sizeof(int))) != cudaSuccess) return fail(e);
+            if ((e = cudaMemcpy(fp->grp_e, grp_e.data(), grp_e.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+            fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, fp->grp_off, fp->grp_e, (int)btiles.size(), pw_max, ne_max, nbuf, ntb};
+            fp->belt_slack = bv.slack;
             fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true; fp->belt_tiles_per_ring = N / T;
             // latitude chunks: the tile list runs from ring 2N down to the first belt ring, N / T tiles per ring
             {

@@ -47,9 +47,11 @@ struct BeltDev {
     const int *pair_off;
     const int *woff;          // per pair entry: offset (in float2, even) of its tap array within a tap buffer
     const int4 *tiles;        // (ring, k0, slot, number of input rings)
+    const int *grp_off;       // per slot: its group boundaries are grp_e[grp_off[slot] .. grp_off[slot + 1])
+    const int *grp_e;         // entry indices (relative to the ring's first entry) where the groups begin, then the end
     int ntiles;
     int pw_max;               // float2 entries of a tap buffer
-    int ne_max;               // input rings per tile, at most
+    int ne_max;               // input rings per group, at most
     int nbuf;                 // stage buffers
     int ntb;                  // tap buffers (1 or 2)
 };

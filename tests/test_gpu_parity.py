@@ -151,8 +151,7 @@ def test_config5_sampled_batch3(sc):
 
 def test_config6_paper_scale_sampled(sc):
     """The paper's own operating point (theta_cut 240', ~61,000 neighbours per pixel): counts
-    and values on 300 sampled pixels.  The belt tap arrays do not fit at this disc size, so the sym kernel
-    (two accumulator sets) covers the belt as well."""
+    and values on 300 sampled pixels.  The belt kernel streams its taps in ring groups at this disc size."""
     cfg = gen.config(6)
     T, maps = gen.table_for(cfg), gen.maps_for(cfg)
     sel = gen.sample_pixels(cfg.nside, 300, seed=66)
