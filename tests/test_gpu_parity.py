@@ -378,6 +378,23 @@ def test_profile_entry_and_partition(sc):
         assert ms["generic_warp_kernel"] > 0.1 and ms["belt_kernel"] < 0.01 and ms["sym_kernel"] < 0.01
 
 
+@pytest.mark.parametrize("ci,B", [(3, 1), (3, 5), (2, 2)])
+def test_host_entry_pipelined_chunks(sc, ci, B):
+    """sc_convolve_host (latitude chunks on three streams, belt + cap kernels launched per chunk) returns
+    exactly what sc_convolve computes, also when B exceeds the maps per launch."""
+    cfg = gen.config(ci)
+    T = gen.table_for(cfg)
+    maps = [gen.noise_map(cfg.npix, 700 + 10 * ci + b) for b in range(B)]
+    with sc.Plan(cfg.nside, T, cfg.theta_max, B) as plan:
+        dev = _gpu_convolve(sc, plan, maps)
+        host = plan.convolve_host(maps)
+        host2 = plan.convolve_host(maps)                      # event pool reuse
+        assert sc.sc_last_launch_count(plan.handle) > 3
+    for b in range(B):
+        np.testing.assert_array_equal(host[b], dev[b])
+        np.testing.assert_array_equal(host2[b], dev[b])
+
+
 def test_knife_edge_host_adjudication(sc, monkeypatch):
     """Widen the knife-edge band so that many pairs are decided on the host with the host libm;
     sets must still equal the oracle's and the override list must be in use."""
