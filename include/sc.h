@@ -80,6 +80,8 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
  *   B          >= 1.
  *   cuda_stream  a cudaStream_t (CUstream) passed as void*; NULL = the legacy default stream.
  * Map values are plain numbers: no bad-pixel sentinel is interpreted (paper silent).
+ * Only kernel launches are enqueued (no allocation, no host synchronisation), so the call may be
+ * captured into a CUDA graph.
  */
 sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *const *out_maps,
                       int B, void *cuda_stream);
