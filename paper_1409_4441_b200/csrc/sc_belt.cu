@@ -16,6 +16,8 @@
 // There is no block-wide barrier after the prologue.
 #include "sc_fast.cuh"
 
+#include <type_traits>
+
 #ifndef SC_BELT_PREFETCH
 #define SC_BELT_PREFETCH 0
 #endif
@@ -172,7 +174,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     const int wo = F.woff[e0 + e];
                     int delta, w0a, a0, ng;
                     belt_window(pe, sh, k0, delta, w0a, a0, ng);
-                    if (pt == 0) desc[e - ge0] = make_int4(ng, wo * 8, 2 * pe.hw + 1, 0);
+                    if (pt == 0) desc[e - ge0] = make_int4(ng, wo * 8, 2 * pe.hw + 1, a0);
                     // nearest pixel of ring rq in azimuth: kc = k + delta, at angle dcc from p.  In the belt
                     // Y = N (2k + 1 - sh + shq), so delta = (1 - sh + shq) >> 1 and the remainder is N or 0.
                     const int Yk = 1 - sh + pe.shq;
@@ -265,25 +267,54 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                         }
                     }
                 };
-                const int ng = d.x;
-#if SC_BELT_PREFETCH
-                load_chunk(0, tp[0], mv[0]);
-#pragma unroll 1
-                for (int g4 = 0; g4 < ng; g4 += 2) {
-                    if (g4 + 1 < ng) load_chunk(g4 + 1, tp[1], mv[1]);
-                    fma_chunk(tp[0], mv[0]);
-                    if (g4 + 1 < ng) {
-                        if (g4 + 2 < ng) load_chunk(g4 + 2, tp[0], mv[0]);
-                        fma_chunk(tp[1], mv[1]);
+                // Edge chunks.  With q = 4 g4 + p - a0 the tap pair of pixels (0,1) at chunk position p is
+                // non-zero only for 0 <= q <= 2hw + 1 and that of pixels (2,3) only for 2 <= q <= 2hw + 3, so
+                // the first and the last chunk of a ring run a body WITHOUT the FFMA2s that would multiply two
+                // zero taps (compile-time masks, selected by a warp-uniform switch on the alignment).
+                auto fma_masked = [&](const float4 (&t)[3], const float4 (&m)[8], auto M01, auto M23) {
+                    constexpr int k01 = decltype(M01)::value, k23 = decltype(M23)::value;
+                    const float2 pwr[6] = {make_float2(t[0].x, t[0].y), make_float2(t[0].z, t[0].w), make_float2(t[1].x, t[1].y),
+                                           make_float2(t[1].z, t[1].w), make_float2(t[2].x, t[2].y), make_float2(t[2].z, t[2].w)};
+#pragma unroll
+                    for (int g = 0; g < 8; ++g) {
+                        const float mm[4] = {m[g].x, m[g].y, m[g].z, m[g].w};
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const float2 m2 = make_float2(mm[i], mm[i]);
+                            if ((k01 >> i) & 1) acc01[g] = __ffma2_rn(pwr[2 + i], m2, acc01[g]);
+                            if ((k23 >> i) & 1) acc23[g] = __ffma2_rn(pwr[i], m2, acc23[g]);
+                        }
                     }
+                };
+#define SC_MASKS(a, b) std::integral_constant<int, a>{}, std::integral_constant<int, b>{}
+                const int ng = d.x, a0 = d.w;
+                const int rem = a0 + d.z + 3 - 4 * (ng - 1);              // valid positions of the last chunk, 1 .. 4
+                int g4 = 0, gend = ng;
+                if (ng >= 2) {
+                    load_chunk(0, tp[0], mv[0]);
+                    switch (a0) {                                         // pixels (0,1): p >= a0; pixels (2,3): p >= a0 + 2
+                        case 0: fma_masked(tp[0], mv[0], SC_MASKS(0xF, 0xC)); break;
+                        case 1: fma_masked(tp[0], mv[0], SC_MASKS(0xE, 0x8)); break;
+                        case 2: fma_masked(tp[0], mv[0], SC_MASKS(0xC, 0x0)); break;
+                        default: fma_masked(tp[0], mv[0], SC_MASKS(0x8, 0x0)); break;
+                    }
+                    g4 = 1; gend = ng - 1;
                 }
-#else
 #pragma unroll 1
-                for (int g4 = 0; g4 < ng; ++g4) {
+                for (; g4 < gend; ++g4) {
                     load_chunk(g4, tp[0], mv[0]);
                     fma_chunk(tp[0], mv[0]);
                 }
-#endif
+                if (ng >= 2) {
+                    load_chunk(ng - 1, tp[0], mv[0]);
+                    switch (rem) {                                        // pixels (0,1): p <= rem - 3; pixels (2,3): p <= rem - 1
+                        case 1: fma_masked(tp[0], mv[0], SC_MASKS(0x0, 0x1)); break;
+                        case 2: fma_masked(tp[0], mv[0], SC_MASKS(0x0, 0x3)); break;
+                        case 3: fma_masked(tp[0], mv[0], SC_MASKS(0x1, 0x7)); break;
+                        default: fma_masked(tp[0], mv[0], SC_MASKS(0x3, 0xF)); break;
+                    }
+                }
+#undef SC_MASKS
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
                 if (++buf == NBUF) { buf = 0; par ^= 1u; }
