@@ -25,6 +25,7 @@
 #include <cstring>
 #include <map>
 #include <memory>
+#include <type_traits>
 #include <vector>
 
 namespace sc {
@@ -282,13 +283,19 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 #pragma unroll
                 for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
                 float2 jf = f2((float)(-pe.hw));
-                const int pend = i0 + pe.hw + R - 1;
-#pragma unroll 2
-                for (int pos = i0 - pe.hw; pos <= pend; ++pos) {
+                const int pos0 = i0 - pe.hw, pend = i0 + pe.hw + R - 1;
+                // One window position for the pixels rr in MASK (compile time).  The window of the thread is the
+                // union of its R pixels' windows, which are one position apart: pixel rr can only be inside the
+                // disc at positions pos0 + rr .. pend - (R - 1 - rr) (host: hw = floor(H / dphi' + 1/2 + 3 rho1),
+                // |dcr0| <= dphi' / 2, pixel rr is centred rr (1 +- rho1) positions further), so the first and the
+                // last R - 1 positions run bodies without the other pixels' geometry, gather and FMAs.
+                auto body = [&](int pos, auto MASK) {
+                    constexpr int mask = decltype(MASK)::value;
                     float tp[2 * RP];
                     unsigned cb[2 * RP];
 #pragma unroll
                     for (int h = 0; h < RP; ++h) {
+                        if (!((mask >> (2 * h)) & 3)) continue;
                         const float2 d = __ffma2_rn(jf, dphi2, dc2[h]);
                         const float2 y = __fmul2_rn(d, d);
                         float2 p = __ffma2_rn(y, c3, c2);
@@ -300,19 +307,20 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     }
                     // cells below the last: plain lookup; beyond the zero cell: clamp onto it (weight 0);
                     // the last cell and the zero cell (t in [tmax - 1, tmax + 1)) take the branch
-                    unsigned mn = cb[0] - thresh;
+                    unsigned mn = 0xFFFFFFFFu;
 #pragma unroll
-                    for (int rr = 1; rr < R; ++rr) mn = min(mn, cb[rr] - thresh);
+                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) mn = min(mn, cb[rr] - thresh);
 #pragma unroll
-                    for (int rr = 0; rr < R; ++rr) cb[rr] = min(cb[rr], thresh + 1u);
+                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) cb[rr] = min(cb[rr], thresh + 1u);
                     if (mn < 2u) {
 #pragma unroll
                         for (int rr = 0; rr < R; ++rr)
-                            if (cb[rr] >= thresh) slow(rr, tp[rr], cb[rr], pos);
+                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], cb[rr], pos);
                     }
                     float K[R];
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) {
+                        if (!((mask >> rr) & 1)) continue;
                         float2 el;                                  // tab[cb - kMagicBits], one LEA for the address
                         asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + cb[rr] * 8u));
                         K[rr] = fmaf(tp[rr], el.y, el.x);
@@ -324,6 +332,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         const float2 m01 = f2(mn4.x, mn4.y), m23 = f2(mn4.z, mn4.w), m45 = f2(ms4.x, ms4.y), m67 = f2(ms4.z, ms4.w);
 #pragma unroll
                         for (int rr = 0; rr < R; ++rr) {
+                            if (!((mask >> rr) & 1)) continue;
                             const float2 Kd = f2(K[rr]);
                             acc[rr][b][0] = __ffma2_rn(Kd, m01, acc[rr][b][0]);
                             acc[rr][b][1] = __ffma2_rn(Kd, m23, acc[rr][b][1]);
@@ -332,6 +341,20 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         }
                     }
                     jf = __fadd2_rn(jf, f2(1.0f));
+                };
+                constexpr int kAll = (1 << R) - 1;
+                int pos = pos0, plast = pend;
+                const bool peel = R > 1 && 2 * pe.hw >= R - 2;       // first and last R - 1 positions do not overlap
+                if (peel) {
+                    body(pos++, std::integral_constant<int, 1>{});
+                    if (R == 4) { body(pos++, std::integral_constant<int, 3>{}); body(pos++, std::integral_constant<int, 7>{}); }
+                    plast = pend - (R - 1);
+                }
+#pragma unroll 2
+                for (; pos <= plast; ++pos) body(pos, std::integral_constant<int, kAll>{});
+                if (peel) {
+                    if (R == 4) { body(pos++, std::integral_constant<int, 14 & kAll>{}); body(pos++, std::integral_constant<int, 12 & kAll>{}); }
+                    body(pos++, std::integral_constant<int, (1 << (R - 1))>{});
                 }
                 if (TOT) {
 #pragma unroll
