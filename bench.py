@@ -310,6 +310,71 @@ def run_ours(args, cfg, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_bands(args, cfg, rank, world, local_rank):
+    """Strong scaling (optional mode, not the driver's default): the SAME maps on every rank, each rank
+    convolves its latitude band after a halo exchange of the overlap rows.  One JSON line
+    with "scaling": "strong"; value = pairs of the whole map(s) / max time over ranks."""
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    import paper_1409_4441_b200 as sc
+    from paper_1409_4441_b200 import dist as scdist
+    T = gen.table_for(cfg)
+    host_maps = gen.maps_for(cfg)
+    B = len(host_maps)
+    plan = sc.Plan(cfg.nside, T, cfg.theta_max, B)
+    total_pairs = plan.info()["total_pairs"]
+    bands = [plan.band(world, r) for r in range(world)]
+    mine = bands[rank]
+    # this rank owns the rows of its band only; the overlap arrives by the halo exchange in every step
+    dev_in = [torch.zeros(cfg.npix, dtype=torch.float32, device="cuda") for _ in range(B)]
+    for m, h in zip(dev_in, host_maps):
+        for lo, hi in scdist._ranges(mine["out_rows"]):
+            m[lo:hi] = torch.from_numpy(h[lo:hi]).cuda()
+    dev_out = [torch.zeros_like(m) for m in dev_in]
+
+    def step():
+        if world > 1:
+            scdist.exchange_halos(dev_in, bands, rank)
+        plan.convolve_band(mine["ring_lo"], mine["ring_hi"], dev_in, dev_out)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank); sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.result()
+    (total_ms,), _ = scdist.combine_timing([e0.elapsed_time(e1)], 0)
+    if rank == 0:
+        value = total_pairs * B * args.steps / (total_ms * 1e-3)
+        halo = sum(hi - lo for lo, hi in scdist._subtract(scdist._ranges(mine["in_rows"]), scdist._ranges(mine["out_rows"])))
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": _workload_name(cfg), "mode": "latitude bands + halo exchange",
+                                     "band_of_rank0": mine, "halo_bytes_per_step_rank0": 4 * halo * B},
+                          "map_convs_per_s": B * args.steps / (total_ms * 1e-3), "clocks": clocks,
+                          "gpu_launches": args.steps * sc.sc_last_launch_count(plan.handle)}), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -318,6 +383,9 @@ def main():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number (1-5); 6 = paper-scale theta_cut 240' (context)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", default="auto", choices=["auto", "generic"])
+    ap.add_argument("--bands", action="store_true",
+                    help="strong scaling: ONE batch of maps split into latitude bands over the ranks "
+                         "(halo exchange + sc_convolve_band) instead of independent maps per rank")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
@@ -328,6 +396,8 @@ def main():
     cfg = gen.config(args.config)
     if args.impl == "reference":
         run_reference(args, cfg, rank, world)
+    elif args.bands:
+        run_bands(args, cfg, rank, world, local_rank)
     else:
         run_ours(args, cfg, rank, world, local_rank)
 

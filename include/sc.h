@@ -163,8 +163,8 @@ sc_status sc_plan_partition(const sc_plan *plan, int *polar_rings, int *first_be
  * A band is a range of BASE rings lo .. hi (1 <= lo <= hi <= 2 nside) together with the southern mirror
  * rings 4 nside - hi .. 4 nside - lo, because the kernels evaluate a pair geometry once for both.
  *
- * sc_band_partition -- band `rank` of a split of the sphere into `world` bands of nearly equal pixel
- * counts (1 <= world <= 2 nside).  HOST outputs, any may be NULL:
+ * sc_band_partition -- band `rank` of a split of the sphere into `world` bands of nearly equal estimated
+ * work (cap pixels cost more than belt pixels; 1 <= world <= 2 nside).  HOST outputs, any may be NULL:
  *   ring_lo, ring_hi   the band's base rings
  *   out_rows[4]        pixel ranges [o0, o1) U [o2, o3) the band's convolution writes
  *   in_rows[4]         pixel ranges [i0, i1) U [i2, i3) it reads (band + theta_max overlap); a range may be

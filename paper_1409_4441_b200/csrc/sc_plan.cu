@@ -551,8 +551,17 @@ sc_status sc_band_partition(const sc_plan *plan, int world, int rank, int *ring_
     if (!plan) return SC_ERR_INVALID_ARG;
     const int N = plan->dev.nside;
     if (world < 1 || world > 2 * N || rank < 0 || rank >= world) return SC_ERR_INVALID_ARG;
-    // base ring r stands for rings r and 4N - r: 2 n_r pixels (n_r for the equator ring 2N)
-    const int64_t total = plan->dev.npix;
+    // base ring r stands for rings r and 4N - r: 2 n_r pixels (n_r for the equator ring 2N).  Bands get
+    // nearly equal ESTIMATED WORK: a cap pixel (sym kernel) costs about 3.3 belt pixels (stencil) and a pixel
+    // next to the poles (warp-per-pixel kernel) about 65 (measured ratios, configs 4 and 5).
+    const int pr = plan->fast ? plan->polar_rings : 0;
+    const int fb = plan->fast ? sc::fast_first_belt_ring(plan->fast) : 2 * N + 1;
+    auto weight = [&](int r) -> int64_t {
+        const int64_t px = (int64_t)plan->rings[r - 1].n * (r < 2 * N ? 2 : 1);
+        return px * (r <= pr ? 200 : (r < fb ? 10 : 3));
+    };
+    int64_t total = 0;
+    for (int r = 1; r <= 2 * N; ++r) total += weight(r);
     auto first_ring = [&](int k) -> int {            // first base ring of band k (band `world` starts at 2N + 1)
         if (k <= 0) return 1;
         if (k >= world) return 2 * N + 1;
@@ -560,7 +569,7 @@ sc_status sc_band_partition(const sc_plan *plan, int world, int rank, int *ring_
         int r = 1;
         for (; r <= 2 * N; ++r) {
             if (cum * world >= total * k) break;
-            cum += (int64_t)plan->rings[r - 1].n * (r < 2 * N ? 2 : 1);
+            cum += weight(r);
         }
         // every band keeps at least one ring
         return std::min(std::max(r, k + 1), 2 * N - (world - 1 - k));
