@@ -395,6 +395,34 @@ def test_host_entry_pipelined_chunks(sc, ci, B):
         np.testing.assert_array_equal(host2[b], dev[b])
 
 
+def test_table_too_large_for_shared_memory_falls_back_to_generic(sc):
+    """A 40,000-node table (320 KB of cells) does not fit the fast kernels' shared memory: the plan has no
+    fast path, every entry point still works (generic kernel) and matches the oracle."""
+    nside, theta, ntab = 64, 4.0 * gen.DEG, 40000
+    npix = 12 * nside * nside
+    _, th = gen.table_nodes(theta, ntab)
+    T = np.exp(-2.0 * (th / theta) ** 2) * np.cos(6.0 * th / theta)
+    maps = [gen.noise_map(npix, 77), gen.noise_map(npix, 78)]
+    ref, cnt, sig = O.convolve(nside, T, theta, maps)
+    with sc.Plan(nside, T, theta, 2) as plan:
+        part = plan.partition()
+        assert part["polar_rings"] == 2 * nside and part["first_belt_ring"] == 2 * nside + 1
+        _check_counts(sc, plan, cnt, sig)
+        out = _gpu_convolve(sc, plan, maps)
+        host = plan.convolve_host(maps)
+        import torch
+        dm = [torch.from_numpy(m).cuda() for m in maps]
+        band_out = [torch.full_like(d, float("nan")) for d in dm]
+        for rank in range(3):
+            bd = plan.band(3, rank)
+            plan.convolve_band(bd["ring_lo"], bd["ring_hi"], dm, band_out)
+        torch.cuda.synchronize()
+    for b in range(2):
+        _check_values(out[b], ref[b], f"large table map{b}")
+        np.testing.assert_array_equal(host[b], out[b])
+        np.testing.assert_array_equal(band_out[b].cpu().numpy(), out[b])
+
+
 def test_cuda_graph_capture(sc):
     """sc_convolve only enqueues kernels on the caller's stream (no allocation, no host sync), so it can be
     captured into a CUDA graph and replayed; the replay gives the same bits."""
