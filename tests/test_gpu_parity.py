@@ -395,6 +395,41 @@ def test_host_entry_pipelined_chunks(sc, ci, B):
         np.testing.assert_array_equal(host2[b], dev[b])
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_random_shapes_against_oracle(sc, seed):
+    """Seeded random (Nside, theta_max, table size, batch): every pixel against the oracle (sets and values),
+    and the host entry / latitude bands bit-identical to sc_convolve."""
+    import torch
+    rng = np.random.default_rng(9000 + seed)
+    nside = int(rng.choice([3, 7, 31, 100, 128, 200, 256, 300]))
+    npix = 12 * nside * nside
+    pix = np.sqrt(4 * np.pi / npix)
+    theta = float(min(np.pi / 2, pix * rng.uniform(0.3, 9.0)))
+    ntab = int(rng.choice([2, 17, 1000, 4096, 16384]))
+    B = int(rng.choice([1, 1, 2, 3, 5]))
+    _, th = gen.table_nodes(theta, ntab)
+    T = np.exp(-2.5 * (th / theta) ** 2) * np.cos(rng.uniform(0, 6) * th / theta) + 0.02
+    maps = [gen.noise_map(npix, 9100 + 10 * seed + b) for b in range(B)]
+    ref, cnt, sig = O.convolve(nside, T, theta, maps)
+    with sc.Plan(nside, T, theta, B) as plan:
+        assert plan.info()["total_pairs"] == int(cnt.sum())
+        _check_counts(sc, plan, cnt, sig)
+        dm = [torch.from_numpy(m).cuda() for m in maps]
+        out = plan.convolve(dm)
+        host = plan.convolve_host(maps)
+        band_out = [torch.full_like(d, float("nan")) for d in dm]
+        world = int(rng.integers(1, 6))
+        for rank in range(world):
+            bd = plan.band(world, rank)
+            plan.convolve_band(bd["ring_lo"], bd["ring_hi"], dm, band_out)
+        torch.cuda.synchronize()
+    for b in range(B):
+        got = out[b].cpu().numpy()
+        _check_values(got, ref[b], f"random shape seed {seed}: nside {nside} theta/pix {theta / pix:.2f} ntab {ntab} B {B}")
+        np.testing.assert_array_equal(host[b], got)
+        np.testing.assert_array_equal(band_out[b].cpu().numpy(), got)
+
+
 def test_table_too_large_for_shared_memory_falls_back_to_generic(sc):
     """A 40,000-node table (320 KB of cells) does not fit the fast kernels' shared memory: the plan has no
     fast path, every entry point still works (generic kernel) and matches the oracle."""
