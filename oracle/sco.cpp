@@ -113,6 +113,32 @@ inline double kernel_eval(const double *T, int n, double c, double x) {
     return T[i] + f * (T[i + 1] - T[i]);
 }
 
+/* Two-zone table (reading R11 of PAPER.md:106 "half the available interpolation nodes within the
+ * first 1/16 of the available support"): n nodes (n even, >= 4), h = n/2, x1 = cos(zone_frac * theta_max).
+ * Nodes i = 0 .. h-1 (outer zone):  x_i = c + i (x1 - c) / h;  nodes i = h .. n-1 (inner zone, next to
+ * theta = 0):  x_i = x1 + (i - h)(1 - x1) / (h - 1).  Linear interpolation in x between adjacent nodes. */
+inline double kernel_eval_zoned(const double *T, int n, double c, double x1, double x) {
+    if (x > 1.0) x = 1.0;
+    const int h = n / 2;
+    long i;
+    double f;
+    if (x >= x1) {
+        const double s = (x - x1) / (1.0 - x1) * (double)(h - 1);
+        i = (long)std::floor(s);
+        if (i < 0) i = 0;
+        if (i > h - 2) i = h - 2;
+        f = s - (double)i;
+        i += h;
+    } else {
+        const double s = (x - c) / (x1 - c) * (double)h;
+        i = (long)std::floor(s);
+        if (i < 0) i = 0;
+        if (i > h - 1) i = h - 1;
+        f = s - (double)i;
+    }
+    return T[i] + f * (T[i + 1] - T[i]);
+}
+
 inline int64_t floordiv(int64_t a, int64_t b) { int64_t q = a / b, r = a % b; return (r != 0 && ((r < 0) != (b < 0))) ? q - 1 : q; }
 inline int64_t posmod(int64_t a, int64_t n) { int64_t r = a % n; return r < 0 ? r + n : r; }
 
@@ -247,6 +273,10 @@ double sco_kernel_eval(const double *ktable, int n_table, double theta_max, doub
     return kernel_eval(ktable, n_table, std::cos(theta_max), x);
 }
 
+double sco_kernel_eval_zoned(const double *ktable, int n_table, double theta_max, double zone_frac, double x) {
+    return kernel_eval_zoned(ktable, n_table, std::cos(theta_max), std::cos(zone_frac * theta_max), x);
+}
+
 int sco_neighbours(int nside, double theta_max, int64_t p, int mode,
                    int64_t *buf, int64_t cap, int64_t *n_out) {
     if (nside < 1 || !n_out || !(theta_max > 0.0)) return SCO_ERR_ARG;
@@ -261,11 +291,14 @@ int sco_neighbours(int nside, double theta_max, int64_t p, int mode,
     return SCO_OK;
 }
 
-int sco_convolve(int nside, const double *ktable, int n_table, double theta_max,
-                 const float *const *in, double *const *out, int B,
-                 int64_t n_sel, const int64_t *sel,
-                 int32_t *counts, uint64_t *sigs, int mode, int nthreads) {
+static int convolve_impl(int nside, const double *ktable, int n_table, double theta_max, double zone_frac,
+                         const float *const *in, double *const *out, int B,
+                         int64_t n_sel, const int64_t *sel,
+                         int32_t *counts, uint64_t *sigs, int mode, int nthreads) {
     if (nside < 1 || B < 0 || !(theta_max > 0.0) || theta_max > M_PI) return SCO_ERR_ARG;
+    const bool zoned = zone_frac > 0.0;
+    if (zoned && (zone_frac >= 1.0 || n_table < 4 || (n_table & 1))) return SCO_ERR_ARG;
+    const double x1 = zoned ? std::cos(zone_frac * theta_max) : 0.0;
     if (B > 0 && (!ktable || n_table < 2 || !in || !out)) return SCO_ERR_ARG;
     if (B > 16) return SCO_ERR_ARG;
     const int64_t npix = 12LL * nside * nside;
@@ -285,7 +318,7 @@ int sco_convolve(int nside, const double *ktable, int n_table, double theta_max,
         auto f = [&](int64_t q, double d) {
             ++cnt; sg += (uint64_t)q;
             if (B > 0) {
-                const double K = kernel_eval(ktable, n_table, c, d);
+                const double K = zoned ? kernel_eval_zoned(ktable, n_table, c, x1, d) : kernel_eval(ktable, n_table, c, d);
                 for (int b = 0; b < B; ++b) sum[b] += K * (double)in[b][q];
             }
         };
@@ -295,6 +328,21 @@ int sco_convolve(int nside, const double *ktable, int n_table, double theta_max,
         if (sigs) sigs[j] = sg;
     }
     return SCO_OK;
+}
+
+int sco_convolve(int nside, const double *ktable, int n_table, double theta_max,
+                 const float *const *in, double *const *out, int B,
+                 int64_t n_sel, const int64_t *sel,
+                 int32_t *counts, uint64_t *sigs, int mode, int nthreads) {
+    return convolve_impl(nside, ktable, n_table, theta_max, 0.0, in, out, B, n_sel, sel, counts, sigs, mode, nthreads);
+}
+
+int sco_convolve_zoned(int nside, const double *ktable, int n_table, double theta_max, double zone_frac,
+                       const float *const *in, double *const *out, int B,
+                       int64_t n_sel, const int64_t *sel,
+                       int32_t *counts, uint64_t *sigs, int mode, int nthreads) {
+    if (!(zone_frac > 0.0)) return SCO_ERR_ARG;
+    return convolve_impl(nside, ktable, n_table, theta_max, zone_frac, in, out, B, n_sel, sel, counts, sigs, mode, nthreads);
 }
 
 int sco_count(int nside, double theta_max, int64_t n_sel, const int64_t *sel,

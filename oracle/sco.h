@@ -18,7 +18,8 @@
  *
  * Pins: tests/test_oracle_*.py (-m "not gpu"): explicit Nside 1 / 2 layouts, brute force vs disc
  * query, exact pair totals, identity limit, constant map -> b_0, zonal eigenfunctions -> b_l,
- * linearity, operator symmetry.  Nothing here is "parity unpinned" except where DESIGN.md says so.
+ * linearity, operator symmetry; two-zone table: equals the uniform table when the zones have equal
+ * spacing, exact for kernels linear in x, node values reproduced.  Nothing here is "parity unpinned" except where DESIGN.md says so.
  */
 #ifndef SCO_H
 #define SCO_H
@@ -48,6 +49,12 @@ int sco_pix2ang(int nside, int64_t n, const int64_t *pix, int32_t *ring, int32_t
  * nodes x_i = c + i (1-c)/(n-1), c = cos(theta_max). */
 double sco_kernel_eval(const double *ktable, int n_table, double theta_max, double x);
 
+/* Two-zone table (reading R11): n_table even >= 4, h = n_table / 2,
+ * x1 = cos(zone_frac * theta_max), 0 < zone_frac < 1.  Nodes i < h: x_i = c + i (x1 - c) / h (outer zone);
+ * nodes i >= h: x_i = x1 + (i - h)(1 - x1) / (h - 1) (inner zone: half the nodes next to theta = 0).
+ * Linear interpolation in x between adjacent nodes. */
+double sco_kernel_eval_zoned(const double *ktable, int n_table, double theta_max, double zone_frac, double x);
+
 /* Neighbour list of one output pixel, ascending ring then ascending in-ring order of visit.
  * buf may be NULL (count only). Returns the count in *n_out (even if > cap). */
 int sco_neighbours(int nside, double theta_max, int64_t p, int mode,
@@ -63,6 +70,12 @@ int sco_convolve(int nside, const double *ktable, int n_table, double theta_max,
                  const float *const *in, double *const *out, int B,
                  int64_t n_sel, const int64_t *sel,
                  int32_t *counts, uint64_t *sigs, int mode, int nthreads);
+
+/* The same convolution with the two-zone table of sco_kernel_eval_zoned. */
+int sco_convolve_zoned(int nside, const double *ktable, int n_table, double theta_max, double zone_frac,
+                       const float *const *in, double *const *out, int B,
+                       int64_t n_sel, const int64_t *sel,
+                       int32_t *counts, uint64_t *sigs, int mode, int nthreads);
 
 /* Count-only pass that locates the two ends of every (pixel, ring) run with the same fp64 test
  * instead of testing every interior pixel (uses: inclusion along a ring is one contiguous arc).

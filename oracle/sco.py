@@ -25,6 +25,9 @@ def load():
         lib.sco_pix2ang.argtypes = [i32, i64] + [vp] * 6
         lib.sco_kernel_eval.argtypes = [vp, i32, dbl, dbl]
         lib.sco_kernel_eval.restype = dbl
+        lib.sco_kernel_eval_zoned.argtypes = [vp, i32, dbl, dbl, dbl]
+        lib.sco_kernel_eval_zoned.restype = dbl
+        lib.sco_convolve_zoned.argtypes = [i32, vp, i32, dbl, dbl, vp, vp, i32, i64, vp, vp, vp, i32, i32]
         lib.sco_neighbours.argtypes = [i32, dbl, i64, i32, vp, i64, vp]
         lib.sco_convolve.argtypes = [i32, vp, i32, dbl, vp, vp, i32, i64, vp, vp, vp, i32, i32]
         lib.sco_count.argtypes = [i32, dbl, i64, vp, vp, vp, i32]
@@ -74,6 +77,11 @@ def kernel_eval(ktable, theta_max, x):
     return load().sco_kernel_eval(_ptr(kt), kt.size, float(theta_max), float(x))
 
 
+def kernel_eval_zoned(ktable, theta_max, zone_frac, x):
+    kt = np.ascontiguousarray(ktable, np.float64)
+    return load().sco_kernel_eval_zoned(_ptr(kt), kt.size, float(theta_max), float(zone_frac), float(x))
+
+
 def neighbours(nside, theta_max, p, mode=MODE_DISC):
     lib = load()
     n = C.c_int64(0)
@@ -86,8 +94,9 @@ def neighbours(nside, theta_max, p, mode=MODE_DISC):
 
 
 def convolve(nside, ktable, theta_max, maps, sel=None, mode=MODE_DISC, nthreads=0,
-             want_counts=True):
-    """maps: sequence of B fp32 arrays (N_pix).  Returns (out[B, n_out] fp64, counts, sigs)."""
+             want_counts=True, zone_frac=None):
+    """maps: sequence of B fp32 arrays (N_pix).  Returns (out[B, n_out] fp64, counts, sigs).
+    zone_frac: None = uniform table in cos(theta); else the two-zone table of sco_kernel_eval_zoned."""
     lib = load()
     maps = [np.ascontiguousarray(m, np.float32) for m in maps]
     B = len(maps)
@@ -103,9 +112,15 @@ def convolve(nside, ktable, theta_max, maps, sel=None, mode=MODE_DISC, nthreads=
     out_ptrs = (C.c_void_p * max(B, 1))(*[out[b].ctypes.data for b in range(max(B, 1))])
     counts = np.zeros(nout, np.int32) if want_counts else None
     sigs = np.zeros(nout, np.uint64) if want_counts else None
-    _chk(lib.sco_convolve(nside, _ptr(kt), 0 if kt is None else kt.size, float(theta_max),
-                          in_ptrs, out_ptrs, B, nout if sel_a is not None else 0, _ptr(sel_a),
-                          _ptr(counts), _ptr(sigs), mode, nthreads), "sco_convolve")
+    if zone_frac is None:
+        _chk(lib.sco_convolve(nside, _ptr(kt), 0 if kt is None else kt.size, float(theta_max),
+                              in_ptrs, out_ptrs, B, nout if sel_a is not None else 0, _ptr(sel_a),
+                              _ptr(counts), _ptr(sigs), mode, nthreads), "sco_convolve")
+    else:
+        _chk(lib.sco_convolve_zoned(nside, _ptr(kt), 0 if kt is None else kt.size, float(theta_max),
+                                    float(zone_frac), in_ptrs, out_ptrs, B,
+                                    nout if sel_a is not None else 0, _ptr(sel_a),
+                                    _ptr(counts), _ptr(sigs), mode, nthreads), "sco_convolve_zoned")
     return out[:B], counts, sigs
 
 

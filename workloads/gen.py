@@ -137,6 +137,19 @@ def table_nodes(theta_max: float, n: int):
     return x, theta
 
 
+def zoned_table_nodes(theta_max: float, n: int, zone_frac: float):
+    """Nodes of the two-zone table (reading R11): n even, h = n / 2,
+    x1 = cos(zone_frac theta_max); x_i = c + i (x1 - c) / h for i < h, x_i = x1 + (i - h)(1 - x1)/(h - 1)
+    for i >= h.  -> (x_i, theta_i = acos x_i); x_0 = cos(theta_max), x_{n-1} = 1."""
+    if n < 4 or n % 2 or not (0.0 < zone_frac < 1.0):
+        raise ValueError("n even >= 4 and 0 < zone_frac < 1")
+    h = n // 2
+    c, x1 = np.cos(theta_max), np.cos(zone_frac * theta_max)
+    x = np.concatenate([c + np.arange(h) * (x1 - c) / h, x1 + np.arange(h) * (1.0 - x1) / (h - 1)])
+    x[-1] = 1.0
+    return x, np.arccos(np.clip(x, -1.0, 1.0))
+
+
 def gaussian_table(fwhm: float, theta_max: float, n: int) -> np.ndarray:
     """K(theta) = exp(-theta^2 / 2 sigma^2), sigma = FWHM / 2.3548 (as BASELINE.json writes it;
     'Gaussian beam with a given FWHM', PAPER.md:86)."""
