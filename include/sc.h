@@ -71,6 +71,20 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
                          int n_table, double theta_max, int max_batch);
 
 /*
+ * sc_plan_create_zoned -- the same with the paper-style two-zone table ("we place half the
+ * available interpolation nodes within the first 1/16 of the available support"; reading R11).
+ *   n_table    even, >= 4; h = n_table / 2.
+ *   zone_frac  0 < zone_frac < 1 (the paper: 1/16); x1 = cos(zone_frac * theta_max).  0 = uniform table.
+ *   ktable     K at the nodes  x_i = c + i (x1 - c) / h            for i <  h  (outer zone),
+ *                              x_i = x1 + (i - h)(1 - x1) / (h - 1) for i >= h  (inner zone, next to theta = 0),
+ *              linear interpolation in x = cos(theta) between adjacent nodes.
+ * The inner zone must be at least as dense as the outer one ((h - 1)/(1 - x1) >= h/(x1 - c)), otherwise
+ * SC_ERR_INVALID_ARG.  Everything else as sc_plan_create.
+ */
+sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const double *ktable,
+                               int n_table, double theta_max, double zone_frac, int max_batch);
+
+/*
  * sc_convolve -- the hot path.  Enqueues the convolution of B maps on `cuda_stream` and returns
  * without synchronising the host.
  *   in_maps    HOST array of B DEVICE pointers, each to N_pix fp32 values (RING order),

@@ -13,7 +13,7 @@ SC_PATH_AUTO, SC_PATH_GENERIC = 0, 1
 SC_K_POLAR, SC_K_SYM, SC_K_BELT, SC_K_COUNT = 0, 1, 2, 3
 KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
 
-EXPORTS = ("sc_plan_create", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
+EXPORTS = ("sc_plan_create", "sc_plan_create_zoned", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
            "sc_band_partition", "sc_convolve_band",
            "sc_plan_destroy", "sc_plan_set_path",
            "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_last_launch_count",
@@ -41,6 +41,7 @@ def lib():
         l = C.CDLL(path)
         vp, i32, dbl = C.c_void_p, C.c_int, C.c_double
         l.sc_plan_create.argtypes = [C.POINTER(vp), i32, i32, vp, i32, dbl, i32]
+        l.sc_plan_create_zoned.argtypes = [C.POINTER(vp), i32, i32, vp, i32, dbl, dbl, i32]
         l.sc_convolve.argtypes = [vp, vp, vp, i32, vp]
         l.sc_convolve_host.argtypes = [vp, vp, vp, i32]
         l.sc_convolve_profile.argtypes = [vp, vp, vp, i32, vp, vp]
@@ -75,6 +76,16 @@ def sc_plan_create(nside, ordering, ktable, theta_max, max_batch=1):
     h = C.c_void_p(None)
     _chk(lib().sc_plan_create(C.byref(h), int(nside), int(ordering), kt.ctypes.data_as(C.c_void_p),
                               int(kt.size), float(theta_max), int(max_batch)), "sc_plan_create")
+    return h.value
+
+
+def sc_plan_create_zoned(nside, ordering, ktable, theta_max, zone_frac, max_batch=1):
+    """Two-zone table (include/sc.h): ktable at the zoned nodes, zone_frac in (0, 1)."""
+    kt = np.ascontiguousarray(ktable, np.float64)
+    h = C.c_void_p(None)
+    _chk(lib().sc_plan_create_zoned(C.byref(h), int(nside), int(ordering), kt.ctypes.data_as(C.c_void_p),
+                                    int(kt.size), float(theta_max), float(zone_frac), int(max_batch)),
+         "sc_plan_create_zoned")
     return h.value
 
 
@@ -163,10 +174,13 @@ def sc_last_launch_count(plan):
 class Plan:
     """Convenience owner of a plan for torch users: maps are torch CUDA fp32 tensors."""
 
-    def __init__(self, nside, ktable, theta_max, max_batch=1, ordering=SC_ORDER_RING):
+    def __init__(self, nside, ktable, theta_max, max_batch=1, ordering=SC_ORDER_RING, zone_frac=None):
         self.nside = int(nside)
         self.npix = 12 * self.nside * self.nside
-        self.handle = sc_plan_create(nside, ordering, ktable, theta_max, max_batch)
+        if zone_frac is None:
+            self.handle = sc_plan_create(nside, ordering, ktable, theta_max, max_batch)
+        else:
+            self.handle = sc_plan_create_zoned(nside, ordering, ktable, theta_max, zone_frac, max_batch)
 
     def close(self):
         if getattr(self, "handle", None):

@@ -60,10 +60,18 @@ __device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j
             if (t <= P.tmax + P.eps) {
                 const float2 el = __ldg(&P.tabh[P.ntab - 2]);
                 unc = true;
-                Ku = fmaf(fminf(t, P.tmax) - 0.5f, el.y, el.x);
+                float xk = fminf(t, P.tmax) - 0.5f;
+                if (P.zoned) { int jz; zoned_cell(P, fminf(t, P.tmax), jz, xk); xk -= 0.5f; }   // last cell, centred form
+                Ku = fmaf(xk, el.y, el.x);
             }
             return 0.f;
         }
+    }
+    if (P.zoned) {                                   // two-zone table (t < tmax - eps here)
+        int jz; float fz;
+        zoned_cell(P, tp + 0.5f, jz, fz);
+        const float2 el = __ldg(&P.tabh[jz]);
+        return fmaf(fz - 0.5f, el.y, el.x);
     }
     const float2 el = __ldg(&P.tabh[bits - kMagicBits]);
     return fmaf(tp, el.y, el.x);

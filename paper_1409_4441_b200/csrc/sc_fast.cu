@@ -89,7 +89,8 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 // kSymBuf stage buffers; there is no block-wide barrier after the prologue.
 // TOT: per-step partial sums are added to a second accumulator set (pairwise-like summation; needed for
 // discs of thousands of pixels, costs 8 R B registers).
-template <int B, int R, int NC, bool TOT>
+// Z: two-zone table (lookup at tau(t), R11).
+template <int B, int R, int NC, bool TOT, bool Z>
 __global__ void __launch_bounds__(NC + kSymProd, 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(R == 1 || R == 2 || R == 4, "R");
@@ -260,7 +261,9 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                             const unsigned mask = sym_exact_mask(P, r, ka + rr, ip, pe.rq, kc + pos - i0, pe.ipq, t);
                             if (mask) {
                                 const float2 el = tab[P.ntab - 2];
-                                const float Ku = fmaf(fminf(t, tmax) - 0.5f, el.y, el.x);
+                                float xk = fminf(t, tmax) - 0.5f;
+                                if (Z) { int jz; zoned_cell(P, fminf(t, tmax), jz, xk); xk -= 0.5f; }   // last cell, centred form
+                                const float Ku = fmaf(xk, el.y, el.x);
 #pragma unroll
                                 for (int b = 0; b < B; ++b) {
                                     const unsigned a = pn[b] + 16u * (unsigned)slot_of_pos<R>(pos);
@@ -279,6 +282,10 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 };
 
                 const float2 dphi2 = f2(pe.dphi), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
+                // two-zone table: with t2 = t - 1/2, alpha t - 1/2 = alpha t2 + (alpha - 1)/2 and gamma (t - t1) - 1/2 = gamma t2 + gamma/2 - gamma t1 - 1/2
+                const float2 za2 = f2(P.z_alpha), zao2 = f2(0.5f * P.z_alpha - 0.5f), zg2 = f2(P.z_gamma), zgo2 = f2(0.5f * P.z_gamma - P.z_t1g - 0.5f);
+                const float zhm1f = (float)P.z_hm1;
+                const unsigned zhm1 = (unsigned)P.z_hm1;
                 float2 dc2[RP];
 #pragma unroll
                 for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
@@ -291,8 +298,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 // last R - 1 positions run bodies without the other pixels' geometry, gather and FMAs.
                 auto body = [&](int pos, auto MASK) {
                     constexpr int mask = decltype(MASK)::value;
-                    float tp[2 * RP];
-                    unsigned cb[2 * RP];
+                    float tp[2 * RP], tz_[2 * RP];
+                    unsigned cb[2 * RP], cz[2 * RP];
 #pragma unroll
                     for (int h = 0; h < RP; ++h) {
                         if (!((mask >> (2 * h)) & 3)) continue;
@@ -304,26 +311,39 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         const float2 bb = __fadd2_rn(t2, f2(kMagic));
                         tp[2 * h] = t2.x; tp[2 * h + 1] = t2.y;
                         cb[2 * h] = __float_as_uint(bb.x); cb[2 * h + 1] = __float_as_uint(bb.y);
+                        if (Z) {
+                            // inner zone: alpha t - 1/2; outer zone: gamma (t - t1) - 1/2 RELATIVE to the zone start
+                            // (full resolution where the kernel is steep), cell offset added to the integer bits
+                            const float2 l1 = __ffma2_rn(t2, za2, zao2), l2 = __ffma2_rn(t2, zg2, zgo2);
+                            const bool o0 = l2.x + zhm1f < l1.x, o1 = l2.y + zhm1f < l1.y;
+                            const float2 tz = f2(o0 ? l2.x : l1.x, o1 ? l2.y : l1.y);
+                            const float2 bz = __fadd2_rn(tz, f2(kMagic));
+                            const float2 fz = __fadd2_rn(tz, __fadd2_rn(f2(kMagic), f2(-bz.x, -bz.y)));   // position - 1/2 in the cell
+                            tz_[2 * h] = fz.x; tz_[2 * h + 1] = fz.y;
+                            cz[2 * h] = __float_as_uint(bz.x) + (o0 ? zhm1 : 0u); cz[2 * h + 1] = __float_as_uint(bz.y) + (o1 ? zhm1 : 0u);
+                        }
                     }
                     // cells below the last: plain lookup; beyond the zero cell: clamp onto it (weight 0);
                     // the last cell and the zero cell (t in [tmax - 1, tmax + 1)) take the branch
                     unsigned mn = 0xFFFFFFFFu;
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) mn = min(mn, cb[rr] - thresh);
+                    float *tl = Z ? tz_ : tp;                              // lookup coordinate - 0.5 and its cell bits
+                    unsigned *cl = Z ? cz : cb;
 #pragma unroll
-                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) cb[rr] = min(cb[rr], thresh + 1u);
+                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) cl[rr] = min(cl[rr], thresh + 1u);
                     if (mn < 2u) {
 #pragma unroll
                         for (int rr = 0; rr < R; ++rr)
-                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], cb[rr], pos);
+                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], cl[rr], pos);
                     }
                     float K[R];
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) {
                         if (!((mask >> rr) & 1)) continue;
                         float2 el;                                  // tab[cb - kMagicBits], one LEA for the address
-                        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + cb[rr] * 8u));
-                        K[rr] = fmaf(tp[rr], el.y, el.x);
+                        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + cl[rr] * 8u));
+                        K[rr] = fmaf(tl[rr], el.y, el.x);
                     }
                     const unsigned so = 16u * (unsigned)slot_of_pos<R>(pos);
 #pragma unroll
@@ -513,15 +533,15 @@ struct FastPlan {
     int *grp_off = nullptr, *grp_e = nullptr;
 };
 
-template <int B, int R, int NC, bool TOT>
+template <int B, int R, int NC, bool TOT, bool Z>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st,
                               const SymTile *tiles, int nt) {
     FastDev F{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s};
-    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT, Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, nt);
     if (grid <= 0) return cudaSuccess;
-    sym_kernel<B, R, NC, TOT><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC, TOT, Z><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
@@ -531,10 +551,13 @@ static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev 
     cudaError_t e = cudaErrorInvalidValue;
 #define SC_SYM_CASE(BB, RR)                                                                  \
     if (B == BB && c.R == RR)                                                                \
-        e = c.threads == 256 ? launch_sym<BB, RR, 256, true>(fp, c, P, io, st, tiles, nt)    \
-                             : launch_sym<BB, RR, 128, true>(fp, c, P, io, st, tiles, nt);
+        e = c.threads == 256 ? (P.zoned ? launch_sym<BB, RR, 256, true, true>(fp, c, P, io, st, tiles, nt)    \
+                                        : launch_sym<BB, RR, 256, true, false>(fp, c, P, io, st, tiles, nt))  \
+                             : (P.zoned ? launch_sym<BB, RR, 128, true, true>(fp, c, P, io, st, tiles, nt)    \
+                                        : launch_sym<BB, RR, 128, true, false>(fp, c, P, io, st, tiles, nt));
     if (B == 1 && c.R == 4 && c.threads == 384) {
-        e = launch_sym<1, 4, 384, false>(fp, c, P, io, st, tiles, nt);
+        e = P.zoned ? launch_sym<1, 4, 384, false, true>(fp, c, P, io, st, tiles, nt)
+                    : launch_sym<1, 4, 384, false, false>(fp, c, P, io, st, tiles, nt);
     } else {
         SC_SYM_CASE(1, 1) SC_SYM_CASE(1, 2) SC_SYM_CASE(1, 4)
         SC_SYM_CASE(2, 1) SC_SYM_CASE(2, 2) SC_SYM_CASE(2, 4)

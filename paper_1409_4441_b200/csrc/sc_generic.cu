@@ -90,9 +90,11 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
                         ++cnt; sig += (unsigned long long)(startq + kq);
                     } else {
                         int i = (int)tt;
-                        if (i > P.ntab - 2) i = P.ntab - 2;
+                        float xk = tt;                                  // K = tab[i].x + xk tab[i].y
+                        if (P.zoned) zoned_cell(P, tt, i, xk);
+                        else if (i > P.ntab - 2) i = P.ntab - 2;
                         const float2 e = __ldg(&P.tab[i]);
-                        const float K = fmaf(tt, e.y, e.x);
+                        const float K = fmaf(xk, e.y, e.x);
 #pragma unroll
                         for (int b = 0; b < B; ++b) racc[b] = fmaf(K, __ldg(&io.in[b][startq + kq]), racc[b]);
                     }
@@ -188,9 +190,11 @@ generic_warp_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1) 
             }
             if (in) {
                 int i = (int)tt;
-                if (i > P.ntab - 2) i = P.ntab - 2;
+                float xk = tt;                                  // K = tab[i].x + xk tab[i].y
+                if (P.zoned) zoned_cell(P, tt, i, xk);
+                else if (i > P.ntab - 2) i = P.ntab - 2;
                 const float2 e = __ldg(&P.tab[i]);
-                const float K = fmaf(tt, e.y, e.x);
+                const float K = fmaf(xk, e.y, e.x);
 #pragma unroll
                 for (int b = 0; b < B; ++b) racc[b] = fmaf(K, __ldg(&io.in[b][startq + kq]), racc[b]);
             }

@@ -24,6 +24,7 @@ struct Dev {
     const int *start, *npr;               // first pixel, pixels in ring
     const int *rlo, *rhi;                 // candidate input-ring interval (1-based, inclusive)
     // device interpolation table: K(t) = tab[i].x + t * tab[i].y for t in [i, i+1), t = (1-dot)*scale
+    // (two-zone plans: K = tab[i].x + (tau - i) tab[i].y and tabh[i].x + (tau - i - 1/2) tabh[i].y)
     const float2 *tab;
     // same cells for the half-cell-shifted coordinate t' = t - 1/2 (fast kernel: round(t') = floor(t)):
     // K(t) = tabh[i].x + t' * tabh[i].y
@@ -32,6 +33,9 @@ struct Dev {
     const unsigned long long *ke_key;
     const unsigned char *ke_in;
     int n_ke;
+    // two-zone table (R11): the lookup coordinate is tau = min(z_alpha t, z_beta + z_gamma t), t = (1-dot) scale
+    int zoned, z_hm1;                     // z_hm1 = n/2 - 1: cells of the inner zone
+    float z_alpha, z_gamma, z_t1g;        // inner zone: tau = z_alpha t; outer zone: tau = z_hm1 + z_gamma t - z_t1g
 };
 
 // Audit outputs (plan creation / debug only)
@@ -83,6 +87,20 @@ __device__ __forceinline__ double canonical_dot(const Dev &P, int rp, int kp, in
     const double cd = cos(__dsub_rn(phip, phiq));
     return __dadd_rn(__dmul_rn(P.z[rp - 1], P.z[rq - 1]),
                      __dmul_rn(__dmul_rn(P.s[rp - 1], P.s[rq - 1]), cd));
+}
+
+// Two-zone table: cell j and position f in [0, 1] inside it for table coordinate t (0 <= t <= tmax).  The
+// outer-zone coordinate is formed relative to the zone start so that pairs just outside the inner zone, where
+// the kernel is steep, keep full fp32 resolution (adding the cell offset first would cost 3 digits).
+__device__ __forceinline__ void zoned_cell(const Dev &P, float t, int &j, float &f) {
+    const float w1 = t * P.z_alpha, w2 = fmaf(t, P.z_gamma, -P.z_t1g);
+    const bool outer = w2 + (float)P.z_hm1 < w1;
+    const float w = fmaxf(outer ? w2 : w1, 0.f);
+    const int off = outer ? P.z_hm1 : 0;
+    int i = (int)w;
+    if (i + off > P.ntab - 2) i = P.ntab - 2 - off;
+    j = i + off;
+    f = w - (float)i;
 }
 
 // Exact decision for one pair (slow path).  If `au` is given the pair is also audited.

@@ -209,7 +209,13 @@ const char *sc_version(void) { return "sc 0.2 (sm_100a)"; }
 
 sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *ktable, int n_table,
                          double theta_max, int max_batch) {
+    return sc_plan_create_zoned(plan, nside, ordering, ktable, n_table, theta_max, 0.0, max_batch);
+}
+
+sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const double *ktable, int n_table,
+                               double theta_max, double zone_frac, int max_batch) {
     if (!plan || !ktable || nside < 1 || n_table < 2 || max_batch < 1) return SC_ERR_INVALID_ARG;
+    if (zone_frac != 0.0 && (!(zone_frac > 0.0) || !(zone_frac < 1.0) || n_table < 4 || (n_table & 1))) return SC_ERR_INVALID_ARG;
     if (!(theta_max > 0.0) || !(theta_max <= M_PI / 2)) return SC_ERR_INVALID_ARG;
     if (ordering == SC_ORDER_NESTED) return SC_ERR_UNSUPPORTED;
     if (ordering != SC_ORDER_RING) return SC_ERR_INVALID_ARG;
@@ -239,6 +245,17 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
         const double one_minus_c = 2.0 * std::sin(0.5 * theta_max) * std::sin(0.5 * theta_max);
         D.scale = (double)(n_table - 1) / one_minus_c;
         D.ke_band = std::ldexp(1.0, -50);
+        // two-zone table (R11): node index as a function of t = (1 - x) scale is the minimum of
+        // two lines when the inner zone is the denser one (that is what the mode is for)
+        D.zoned = 0; D.z_hm1 = 0; D.z_alpha = 1.f; D.z_gamma = 1.f; D.z_t1g = 0.f;
+        if (zone_frac > 0.0) {
+            const int h = n_table / 2;
+            const double u1 = 2.0 * std::sin(0.5 * zone_frac * theta_max) * std::sin(0.5 * zone_frac * theta_max);
+            const double t1 = u1 * D.scale, tm = (double)(n_table - 1);
+            const double alpha = (double)(h - 1) / t1, gamma = (double)h / (tm - t1);
+            if (!(alpha >= gamma)) { st = SC_ERR_INVALID_ARG; break; }
+            D.zoned = 1; D.z_hm1 = h - 1; D.z_alpha = (float)alpha; D.z_gamma = (float)gamma; D.z_t1g = (float)(t1 * gamma);
+        }
         if (const char *e = std::getenv("SC_KNIFE_EDGE_BAND")) { const double v = std::atof(e); if (v > 0) D.ke_band = v; }
 
         // ring tables
@@ -273,6 +290,12 @@ sc_status sc_plan_create(sc_plan **plan, int nside, int ordering, const double *
             const double b = t1 - t0, a = t0 - (double)j * b;
             tab[j] = make_float2((float)a, (float)b);
             tabh[j] = make_float2((float)(a + 0.5 * b), (float)b);
+            if (zone_frac > 0.0) {
+                // two-zone table: cell-local form K = T_j + (tau - j) b_j (the cells of the outer zone carry
+                // twice the slope at twice the index: the intercept form would lose a digit to cancellation)
+                tab[j] = make_float2((float)t0, (float)b);
+                tabh[j] = make_float2((float)(t0 + 0.5 * b), (float)b);      // around the cell centre
+            }
         }
         for (size_t j = (size_t)n_table - 1; j < tab.size(); ++j) tab[j] = tabh[j] = make_float2(0.f, 0.f);
 

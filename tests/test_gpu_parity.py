@@ -395,6 +395,60 @@ def test_host_entry_pipelined_chunks(sc, ci, B):
         np.testing.assert_array_equal(host2[b], dev[b])
 
 
+def _zoned_gauss(theta, n, f, fwhm, ripple):
+    x, th = gen.zoned_table_nodes(theta, n, f)
+    sigma = fwhm / 2.3548
+    return np.exp(-0.5 * (th / sigma) ** 2) * (1.0 + ripple * np.cos(9.0 * th / theta))
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("nside,theta_deg,n,f,B", [(64, 3.4, 4096, 1.0 / 16.0, 1), (128, 2.0, 1024, 0.125, 2),
+                                                     (37, 6.0, 64, 0.5, 1), (256, 1.5, 4096, 1.0 / 16.0, 3)])
+def test_two_zone_table_full(sc, path, nside, theta_deg, n, f, B):
+    """Paper-style two-zone table (reading R11): every pixel against the oracle's
+    sco_convolve_zoned, both kernel paths."""
+    theta = theta_deg * gen.DEG
+    npix = 12 * nside * nside
+    T = _zoned_gauss(theta, n, f, 0.6 * theta, 0.3)
+    maps = [gen.noise_map(npix, 8100 + nside + b) for b in range(B)]
+    ref, cnt, sig = O.convolve(nside, T, theta, maps, zone_frac=f)
+    with sc.Plan(nside, T, theta, B, zone_frac=f) as plan:
+        _set_path(sc, plan, path)
+        _check_counts(sc, plan, cnt, sig)
+        out = _gpu_convolve(sc, plan, maps)
+    for b in range(B):
+        _check_values(out[b], ref[b], f"zoned nside {nside} f {f:.3f} n {n}/{path}/map{b}")
+
+
+@pytest.mark.parametrize("ci", [3, 4])
+def test_two_zone_table_sampled_large(sc, ci):
+    """Two-zone table at Nside 1024 / 2048 (sym + belt + polar kernels): sampled pixels; the uniform-table
+    result of the same kernel differs by the table's interpolation error only."""
+    cfg = gen.config(ci)
+    f, n = 1.0 / 16.0, cfg.n_table
+    T = _zoned_gauss(cfg.theta_max, n, f, cfg.fwhm, 0.2)
+    maps = gen.maps_for(cfg)
+    sel = gen.sample_pixels(cfg.nside, 6000, seed=300 + ci)
+    ref, cnt, sig = O.convolve(cfg.nside, T, cfg.theta_max, maps, sel=sel, zone_frac=f)
+    with sc.Plan(cfg.nside, T, cfg.theta_max, 1, zone_frac=f) as plan:
+        c, s = plan.neighbour_counts()
+        np.testing.assert_array_equal(c.cpu().numpy()[sel], cnt)
+        out = _gpu_convolve(sc, plan, maps)
+        host = plan.convolve_host(maps)
+    _check_values(out[0][sel], ref[0], f"zoned cfg{ci}")
+    np.testing.assert_array_equal(host[0], out[0])
+
+
+def test_two_zone_arguments(sc):
+    T = np.ones(16)
+    with pytest.raises(sc.ScError):
+        sc.Plan(8, np.ones(15), 0.2, 1, zone_frac=0.1)          # odd n
+    with pytest.raises(sc.ScError):
+        sc.Plan(8, T, 0.2, 1, zone_frac=1.0)
+    with pytest.raises(sc.ScError):
+        sc.Plan(8, T, 0.2, 1, zone_frac=0.95)                   # inner zone sparser than the outer one
+
+
 @pytest.mark.parametrize("seed", range(8))
 def test_random_shapes_against_oracle(sc, seed):
     """Seeded random (Nside, theta_max, table size, batch): every pixel against the oracle (sets and values),
