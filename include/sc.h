@@ -38,12 +38,12 @@ typedef struct sc_plan sc_plan; /* opaque */
 typedef enum {
     SC_OK = 0,
     SC_ERR_INVALID_ARG = 1, /* NULL where not allowed, nside < 1, n_table < 2, theta_max out of range, B < 1 ... */
-    SC_ERR_UNSUPPORTED = 2, /* NESTED ordering; 12 nside^2 >= 2^31; knife-edge list overflow */
+    SC_ERR_UNSUPPORTED = 2, /* 12 nside^2 >= 2^31; knife-edge list overflow; latitude bands on a NESTED plan */
     SC_ERR_ALLOC = 3,       /* host or device allocation failed */
     SC_ERR_CUDA = 4         /* no device / a CUDA call failed (sc_last_cuda_error() names it) */
 } sc_status;
 
-enum { SC_ORDER_RING = 0, SC_ORDER_NESTED = 1 };
+enum { SC_ORDER_RING = 0, SC_ORDER_NESTED = 1 };   /* NESTED: nside must be a power of two */
 
 /* Which kernels sc_convolve may use (debug / measurement knob; results are the same operation). */
 enum {
@@ -55,7 +55,9 @@ enum {
  * sc_plan_create -- precompute everything that depends only on (nside, kernel, theta_max).
  *   plan       HOST  out: receives the new plan (unchanged on failure).
  *   nside      HEALPix resolution, >= 1, need not be a power of two; 12 nside^2 < 2^31.
- *   ordering   SC_ORDER_RING.  SC_ORDER_NESTED returns SC_ERR_UNSUPPORTED.
+ *   ordering   SC_ORDER_RING, or SC_ORDER_NESTED (nside a power of two): maps passed to sc_convolve /
+ *              sc_convolve_host are then NESTED ordered; the plan owns RING work buffers (2 x min(max_batch, 4)
+ *              maps) and reorders on the device around the same kernels.  Latitude bands need RING.
  *   ktable     HOST  n_table doubles, K sampled at x_i = c + i (1 - c)/(n_table - 1),
  *              c = cos(theta_max), i.e. ktable[0] = K(cos theta_max), ktable[n_table-1] = K(1).
  *              Copied; the caller may free it after the call.
@@ -131,7 +133,8 @@ sc_status sc_plan_info(const sc_plan *plan, int64_t *npix, int64_t *total_pairs,
 /*
  * sc_debug_neighbour_counts -- verification only, not part of the timed path.  For every pixel
  * p writes the number of included neighbours to count_dev[p] and, if sig_dev != NULL, the sum of
- * the neighbours' RING indices to sig_dev[p].  Both DEVICE pointers, N_pix entries.
+ * the neighbours' RING indices to sig_dev[p].  Both DEVICE pointers, N_pix entries (entry p refers to pixel p
+ * in the plan's ordering; the signature sums RING indices also for NESTED plans; NESTED: synchronous).
  * Uses the same inclusion code as sc_convolve.  Asynchronous on cuda_stream.
  */
 sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uint64_t *sig_dev,

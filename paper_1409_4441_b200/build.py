@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libsc.so")
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["sc_plan.cu", "sc_generic.cu", "sc_fast.cu", "sc_belt.cu"]
+SOURCES = ["sc_plan.cu", "sc_generic.cu", "sc_fast.cu", "sc_belt.cu", "sc_nested.cu"]
 HEADERS = [os.path.join(CSRC, "sc_internal.cuh"), os.path.join(CSRC, "sc_fast.cuh"), os.path.join(ROOT, "include", "sc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

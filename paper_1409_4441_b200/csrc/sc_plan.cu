@@ -24,6 +24,9 @@ cudaError_t fast_convolve(FastPlan *fp, const Dev &P, const Maps &io, int B, cud
 int fast_first_belt_ring(const FastPlan *fp);
 cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int which, cudaStream_t st, int *launches, int chunk);
 int fast_chunk_count(const FastPlan *fp, int B, int kind);
+cudaError_t reorder_f32(int nside, int dir, const float *src, float *dst, cudaStream_t st);
+cudaError_t reorder_i32(int nside, int dir, const int *src, int *dst, cudaStream_t st);
+cudaError_t reorder_u64(int nside, int dir, const unsigned long long *src, unsigned long long *dst, cudaStream_t st);
 cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, int lo, int hi, cudaStream_t st, int *launches);
 void fast_chunk_rings(const FastPlan *fp, int B, int kind, int i, int *lo, int *hi);
 bool fast_available(const FastPlan *fp, int B);
@@ -97,6 +100,10 @@ struct sc_plan {
     mutable int last_launches = 0;
     sc::FastPlan *fast = nullptr;
     int polar_rings = 0;                       // rings 1..polar_rings and their southern mirrors use the generic kernel
+    // NESTED plans: the kernels run on plan-owned RING buffers (nest_maps maps in, nest_maps maps out)
+    int nested = 0;
+    mutable float *nest_in = nullptr, *nest_out = nullptr;
+    mutable int nest_maps = 0;
 };
 
 namespace {
@@ -217,8 +224,8 @@ sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const do
     if (!plan || !ktable || nside < 1 || n_table < 2 || max_batch < 1) return SC_ERR_INVALID_ARG;
     if (zone_frac != 0.0 && (!(zone_frac > 0.0) || !(zone_frac < 1.0) || n_table < 4 || (n_table & 1))) return SC_ERR_INVALID_ARG;
     if (!(theta_max > 0.0) || !(theta_max <= M_PI / 2)) return SC_ERR_INVALID_ARG;
-    if (ordering == SC_ORDER_NESTED) return SC_ERR_UNSUPPORTED;
-    if (ordering != SC_ORDER_RING) return SC_ERR_INVALID_ARG;
+    if (ordering != SC_ORDER_RING && ordering != SC_ORDER_NESTED) return SC_ERR_INVALID_ARG;
+    if (ordering == SC_ORDER_NESTED && (nside & (nside - 1))) return SC_ERR_INVALID_ARG;   // NESTED needs a power of two
     if (12LL * nside * nside >= (1LL << 31)) return SC_ERR_UNSUPPORTED;
     if (n_table > (1 << 24)) return SC_ERR_UNSUPPORTED;
     for (int i = 0; i < n_table; ++i) if (!std::isfinite(ktable[i])) return SC_ERR_INVALID_ARG;
@@ -234,6 +241,7 @@ sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const do
     do {
         if (!cuda_ok(cudaGetDevice(&pl->device), "cudaGetDevice")) { st = SC_ERR_CUDA; break; }
         pl->max_batch = max_batch;
+        pl->nested = ordering == SC_ORDER_NESTED;
         const int N = nside, nr = 4 * N - 1;
         sc::Dev &D = pl->dev;
         D.nside = N; D.nrings = nr; D.npix = 12 * N * N; D.ncap = 2 * N * (N - 1);
@@ -316,6 +324,13 @@ sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const do
         cudaError_t ferr = cudaSuccess;
         pl->fast = sc::fast_plan_create(D, z, s, max_batch, &pl->polar_rings, &ferr);
         if (ferr != cudaSuccess) { cuda_ok(ferr, "fast_plan_create"); st = SC_ERR_CUDA; break; }
+        if (pl->nested) {                              // RING work buffers for up to max_batch (<= maps per launch) maps
+            const int nm = std::min(max_batch, sc::kMaxB);
+            const size_t bytes = (size_t)D.npix * 4 * nm;
+            if (!cuda_ok(cudaMalloc((void **)&pl->nest_in, bytes), "cudaMalloc") ||
+                !cuda_ok(cudaMalloc((void **)&pl->nest_out, bytes), "cudaMalloc")) { st = SC_ERR_ALLOC; break; }
+            pl->nest_maps = nm;
+        }
     } while (0);
     if (st != SC_OK) { sc_plan_destroy(pl); return st; }
     *plan = pl;
@@ -328,6 +343,8 @@ sc_status sc_plan_destroy(sc_plan *plan) {
     for (void *p : plan->owned) cudaFree(p);
     if (plan->stage_in) cudaFree(plan->stage_in);
     if (plan->stage_out) cudaFree(plan->stage_out);
+    if (plan->nest_in) cudaFree(plan->nest_in);
+    if (plan->nest_out) cudaFree(plan->nest_out);
     if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
     if (plan->comp_stream) cudaStreamDestroy(plan->comp_stream);
     if (plan->d2h_stream) cudaStreamDestroy(plan->d2h_stream);
@@ -374,10 +391,27 @@ static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps,
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const sc::Dev &D = plan->dev;
     int launches = 0;
+    const size_t npix = (size_t)D.npix;
+    if (plan->nested && plan->nest_maps < std::min(B, sc::kMaxB)) {       // RING work buffers (first use: synchronous)
+        if (plan->nest_in) cudaFree(plan->nest_in);
+        if (plan->nest_out) cudaFree(plan->nest_out);
+        plan->nest_in = plan->nest_out = nullptr; plan->nest_maps = 0;
+        const int nm = std::min(std::max(B, plan->max_batch), sc::kMaxB);
+        if (!cuda_ok(cudaMalloc((void **)&plan->nest_in, npix * 4 * nm), "cudaMalloc")) return SC_ERR_ALLOC;
+        if (!cuda_ok(cudaMalloc((void **)&plan->nest_out, npix * 4 * nm), "cudaMalloc")) return SC_ERR_ALLOC;
+        plan->nest_maps = nm;
+    }
     for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
         const int nb = std::min(sc::kMaxB, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
+        if (plan->nested) {                                                // NESTED -> RING work buffers
+            for (int b = 0; b < nb; ++b) {
+                SC_CUDA(sc::reorder_f32(D.nside, 0, in_maps[b0 + b], plan->nest_in + npix * b, st));
+                io.in[b] = plan->nest_in + npix * b; io.out[b] = plan->nest_out + npix * b;
+            }
+            launches += nb;
+        }
         if (ev) SC_CUDA(cudaEventRecord(ev[0], st));
         if (plan->path == SC_PATH_GENERIC || !sc::fast_available(plan->fast, nb)) {
             SC_CUDA(sc::launch_generic_conv(D, io, nb, 0, D.npix, 0, 0, st));
@@ -395,6 +429,10 @@ static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps,
             int nl = 0;
             SC_CUDA(sc::fast_convolve(plan->fast, D, io, nb, st, &nl, ev ? ev + 2 : nullptr));
             launches += nl;
+        }
+        if (plan->nested) {                                                // RING results -> NESTED outputs
+            for (int b = 0; b < nb; ++b) SC_CUDA(sc::reorder_f32(D.nside, 1, plan->nest_out + npix * b, out_maps[b0 + b], st));
+            launches += nb;
         }
         if (ev) {
             SC_CUDA(cudaEventSynchronize(ev[3]));
@@ -451,7 +489,7 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
     if (!plan->own_stream) SC_CUDA(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
     const sc::Dev &D = plan->dev;
     const int N = D.nside;
-    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && sc::fast_available(plan->fast, std::min(B, sc::kMaxB));
+    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && !plan->nested && sc::fast_available(plan->fast, std::min(B, sc::kMaxB));
     if (!pipelined) {
         std::vector<const float *> in(B); std::vector<float *> out(B);
         for (int b = 0; b < B; ++b) {
@@ -611,6 +649,7 @@ sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float 
     const sc::Dev &D = plan->dev;
     const int N = D.nside;
     if (ring_lo < 1 || ring_hi < ring_lo || ring_hi > 2 * N) return SC_ERR_INVALID_ARG;
+    if (plan->nested) return SC_ERR_UNSUPPORTED;                       // bands are contiguous rows in RING order only
     for (int b = 0; b < B; ++b) {
         if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
         if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return SC_ERR_INVALID_ARG;
@@ -646,8 +685,25 @@ sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float 
 
 sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uint64_t *sig_dev, void *cuda_stream) {
     if (!plan || !count_dev) return SC_ERR_INVALID_ARG;
-    SC_CUDA(sc::launch_generic_count(plan->dev, count_dev, (unsigned long long *)sig_dev, nullptr, (cudaStream_t)cuda_stream));
-    return SC_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!plan->nested) {
+        SC_CUDA(sc::launch_generic_count(plan->dev, count_dev, (unsigned long long *)sig_dev, nullptr, st));
+        return SC_OK;
+    }
+    // NESTED plan: count in RING order into scratch, then reorder (entry p = NESTED pixel p; the signature
+    // stays the sum of the neighbours' RING indices)
+    const size_t npix = (size_t)plan->dev.npix;
+    int *c_ring = nullptr; unsigned long long *s_ring = nullptr;
+    if (!cuda_ok(cudaMalloc((void **)&c_ring, npix * 4), "cudaMalloc")) return SC_ERR_ALLOC;
+    if (sig_dev && !cuda_ok(cudaMalloc((void **)&s_ring, npix * 8), "cudaMalloc")) { cudaFree(c_ring); return SC_ERR_ALLOC; }
+    sc_status rs = SC_OK;
+    if (!cuda_ok(sc::launch_generic_count(plan->dev, c_ring, s_ring, nullptr, st), "count") ||
+        !cuda_ok(sc::reorder_i32(plan->dev.nside, 1, c_ring, count_dev, st), "reorder") ||
+        (sig_dev && !cuda_ok(sc::reorder_u64(plan->dev.nside, 1, s_ring, (unsigned long long *)sig_dev, st), "reorder")) ||
+        !cuda_ok(cudaStreamSynchronize(st), "sync"))
+        rs = SC_ERR_CUDA;
+    cudaFree(c_ring); cudaFree(s_ring);
+    return rs;
 }
 
 }  // extern "C"

@@ -449,6 +449,50 @@ def test_two_zone_arguments(sc):
         sc.Plan(8, T, 0.2, 1, zone_frac=0.95)                   # inner zone sparser than the outer one
 
 
+@pytest.mark.parametrize("nside,theta_deg,B", [(1, 70.0, 1), (4, 30.0, 2), (64, 3.4, 1), (256, 1.5, 5), (1024, 0.5, 1)])
+def test_nested_ordering(sc, nside, theta_deg, B):
+    """SC_ORDER_NESTED plans: NESTED maps in, NESTED maps out.  The device index map nest -> ring is checked
+    against the oracle's independent one (oracle/nested.py) through the results: out_nested[p] must equal the
+    oracle's RING result at nest2ring(p), and the neighbour counts follow the same permutation."""
+    from oracle import nested
+    theta = theta_deg * gen.DEG
+    npix = 12 * nside * nside
+    n2r = nested.nest2ring(nside)
+    _, th = gen.table_nodes(theta, 1024)
+    T = np.exp(-3.0 * (th / theta) ** 2) + 0.1
+    ring_maps = [gen.noise_map(npix, 8800 + nside + b) for b in range(B)]
+    nest_maps = [m[n2r] for m in ring_maps]                    # nest_map[p] = ring_map[nest2ring(p)]
+    sel = None if nside <= 256 else gen.sample_pixels(nside, 4000, seed=9)
+    ref, cnt, sig = O.convolve(nside, T, theta, ring_maps, sel=sel)
+    with sc.Plan(nside, T, theta, B, ordering=sc.SC_ORDER_NESTED) as plan:
+        out = _gpu_convolve(sc, plan, nest_maps)
+        host = plan.convolve_host(nest_maps)
+        c, s = plan.neighbour_counts()
+        c = c.cpu().numpy()
+    inv = np.empty(npix, np.int64)
+    inv[n2r] = np.arange(npix)                                  # ring pixel -> nested pixel
+    pix = np.arange(npix) if sel is None else sel
+    np.testing.assert_array_equal(c[inv[pix]], cnt)
+    for b in range(B):
+        _check_values(out[b][inv[pix]], ref[b], f"nested nside {nside} map{b}")
+        np.testing.assert_array_equal(host[b], out[b])
+    with sc.Plan(nside, T, theta, B) as ring_plan:              # same kernels: bit-identical to the RING plan
+        ring_out = _gpu_convolve(sc, ring_plan, ring_maps)
+    for b in range(B):
+        np.testing.assert_array_equal(out[b], ring_out[b][n2r])
+
+
+def test_nested_arguments(sc):
+    import torch
+    T = np.ones(8)
+    with pytest.raises(sc.ScError):
+        sc.Plan(12, T, 0.2, 1, ordering=sc.SC_ORDER_NESTED)     # not a power of two
+    with sc.Plan(8, T, 0.2, 1, ordering=sc.SC_ORDER_NESTED) as plan:
+        m = torch.zeros(768, device="cuda")
+        with pytest.raises(sc.ScError):
+            sc.sc_convolve_band(plan.handle, 1, 4, [m.data_ptr()], [torch.empty_like(m).data_ptr()])
+
+
 @pytest.mark.parametrize("seed", range(8))
 def test_random_shapes_against_oracle(sc, seed):
     """Seeded random (Nside, theta_max, table size, batch): every pixel against the oracle (sets and values),

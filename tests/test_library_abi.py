@@ -47,7 +47,7 @@ def test_invalid_arguments_rejected_without_gpu():
     assert l.sc_plan_create(C.byref(h), 8, 0, p, 8, 2.0, 1) == INVALID          # theta_max > pi/2
     assert l.sc_plan_create(C.byref(h), 8, 0, None, 8, 0.1, 1) == INVALID       # NULL table
     assert l.sc_plan_create(C.byref(h), 8, 0, p, 8, 0.1, 0) == INVALID          # max_batch
-    assert l.sc_plan_create(C.byref(h), 8, 1, p, 8, 0.1, 1) == UNSUPPORTED      # NESTED
+    assert l.sc_plan_create(C.byref(h), 12, 1, p, 8, 0.1, 1) == INVALID         # NESTED needs a power of two
     assert l.sc_plan_create(C.byref(h), 8, 7, p, 8, 0.1, 1) == INVALID          # unknown ordering
     assert l.sc_plan_create(C.byref(h), 20000, 0, p, 8, 0.1, 1) == UNSUPPORTED  # 12 nside^2 >= 2^31
     assert h.value is None
