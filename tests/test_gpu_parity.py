@@ -395,6 +395,26 @@ def test_host_entry_pipelined_chunks(sc, ci, B):
         np.testing.assert_array_equal(host2[b], dev[b])
 
 
+def test_paper_style_split_kernel(sc):
+    """A real-space kernel from the paper's least-squares split (PAPER.md:29-58 via workloads/splitfit.py: the
+    oscillating, compact part that complements an l-space kernel truncated at l_cut) through the CUDA path:
+    sampled pixels against the oracle."""
+    from workloads import splitfit
+    nside, theta = 256, 4.0 * gen.DEG
+    K_ell = splitfit.gaussian_beam_ell(30 * gen.ARCMIN, 3 * nside - 1)
+    fit = splitfit.split_fit(K_ell, ell_cut=256, theta_cut=theta, n_nodes=512)
+    T = fit["K_hat_theta"]
+    assert np.all(np.isfinite(T)) and np.sum(np.diff(np.sign(T)) != 0) >= 3          # it oscillates (Fig. 4)
+    maps = [gen.noise_map(12 * nside * nside, 4040)]
+    sel = gen.sample_pixels(nside, 8000, seed=41)
+    ref, cnt, sig = O.convolve(nside, T, theta, maps, sel=sel)
+    with sc.Plan(nside, T, theta, 1) as plan:
+        out = _gpu_convolve(sc, plan, maps)
+        c, s = plan.neighbour_counts()
+    np.testing.assert_array_equal(c.cpu().numpy()[sel], cnt)
+    _check_values(out[0][sel], ref[0], "paper-style split kernel")
+
+
 def _zoned_gauss(theta, n, f, fwhm, ripple):
     x, th = gen.zoned_table_nodes(theta, n, f)
     sigma = fwhm / 2.3548
