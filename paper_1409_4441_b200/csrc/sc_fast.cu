@@ -772,7 +772,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     std::vector<BeltVar> bvars;
     {
         const double mean_nb_b = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
-        if (N % 2048 == 0 && mean_nb_b <= 1000.0 && !std::getenv("SC_BELT_NO512")) bvars.push_back({512, 64});
+        if (N % 2048 == 0 && mean_nb_b <= 700.0 && !std::getenv("SC_BELT_NO512")) bvars.push_back({512, 64});
         if (N % 1024 == 0) { bvars.push_back({256, 256}); bvars.push_back({256, 512}); }
         else if (N % 512 == 0) bvars.push_back({128, 256});
     }
@@ -867,9 +867,9 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         std::vector<Cand> cands;
         // 384 consumer threads only come without the second accumulator set (registers): plain fp32
         // running sums, good to ~3e-7 relative rms for discs of a few hundred pixels (measured 2.7e-7 at
-        // 425), so only while the mean disc holds at most 1000 pixels (4.7e-7 measured at 1380)
+        // 425), so only while the mean disc holds at most 700 pixels (4.7e-7 measured at 1380 for a Gaussian, 6.9e-7 at 960 for a cancelling split kernel)
         const double mean_nb = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
-        if (B == 1 && mean_nb <= 1000.0) cands = {{384, 4}, {256, 4}, {256, 2}, {128, 2}};
+        if (B == 1 && mean_nb <= 700.0) cands = {{384, 4}, {256, 4}, {256, 2}, {128, 2}};
         else if (B == 1) cands = {{256, 4}, {256, 2}, {128, 2}};
         else cands = {{256, 2}, {128, 2}, {128, 1}};
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
