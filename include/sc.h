@@ -1,6 +1,6 @@
 /*
- * sc.h -- C ABI of libsc: real-space convolution of a HEALPix RING map with a compact,
- * radially symmetric kernel on one NVIDIA B200 (sm_100a).
+ * sc.h -- C ABI of libsc: real-space convolution of a HEALPix map (RING ordered; NESTED is reordered on
+ * the device) with a compact, radially symmetric kernel on one NVIDIA B200 (sm_100a).
  *
  * The operation (BASELINE.json north_star; the "real-space portion" that the paper runs on the
  * GPU -- PAPER.md:66 section 2, Fig. 1 caption -- i.e. "convolving a ... map with a
@@ -13,7 +13,8 @@
  *     z_p z_q + (s_p s_q) cos(phi_p - phi_q) >= cos(theta_max)
  * evaluated in IEEE double without FMA contraction (the self pair is included); K is the linear
  * interpolant of the caller's table in cos(theta) (PAPER.md:106 speaks of interpolating the
- * real-space kernel from nodes; node placement here is uniform in cos theta, reading R5);
+ * real-space kernel from nodes; node placement here is uniform in cos theta, reading R5, or the paper's
+ * two-zone placement through sc_plan_create_zoned, reading R11);
  * products and sums are fp32 on the device ("single-precision arithmetic in the GPU",
  * PAPER.md:124).
  *
