@@ -90,9 +90,30 @@ __device__ __forceinline__ void belt_window(const PairEnt &pe, int sh, int k0, i
     ng = (2 * pe.hw + 4 + a0 + 3) >> 2;
 }
 
+
+// ---- tensor memory (TMEM) as accumulator storage -------------------------------------------------------------
+// 512 consumer threads leave 104 registers each: the running totals (32 floats per thread) of the
+// two-accumulator summation do not fit next to the 32 per-ring accumulators, so they live in tensor memory:
+// a warp owns the 32 TMEM lanes of its quadrant (warp % 4) and 32 columns (warp / 4); tcgen05.ld / st with the
+// 32x32b shape move one row (lane) x 16 columns per thread.
+__device__ __forceinline__ void tmem_st16(unsigned taddr, const float (&v)[16]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 :: "r"(taddr), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]),
+                    "f"(v[8]), "f"(v[9]), "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15]) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(unsigned taddr, float (&v)[16]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
+                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
+                 : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
 // SLACK: floats per staged plane beyond the tile (window + alignment); TOT: second accumulator set
 // (flushed every >= 48 taps; needed for discs of thousands of pixels, costs 32 registers).
-template <int NC, int SLACK, bool TOT>
+// TM: the second accumulator set lives in tensor memory (512-consumer variant for large discs).
+template <int NC, int SLACK, bool TOT, bool TM>
 __global__ void __launch_bounds__(NC + kBeltProd, 1)
 belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
     constexpr int T = 4 * NC, LP = T + SLACK;
@@ -110,7 +131,14 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
         for (int i = 0; i < 2; ++i) { mbar_init(&tap_full[i], kTapThreads); mbar_init(&tap_empty[i], NC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    __shared__ unsigned s_tmem;
+    if (TM && tid < 32) {                                      // 128 TMEM columns: 4 column groups x 4 lane quadrants
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"(smem_u32(&s_tmem)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (TM) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const int G = gridDim.x, bid = blockIdx.x;
     const int nrows = (F.ntiles + G - 1) / G;
 
@@ -222,6 +250,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
     if (NC == 512) asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
     int buf = 0; unsigned par = 0;
     int tb = 0; unsigned tpar = 0;
+    const unsigned taddr = TM ? s_tmem + ((((unsigned)(tid >> 5) & 3u) * 32u) << 16) + ((unsigned)tid >> 7) * 32u : 0u;
     for (int row = 0; row < nrows; ++row) {
         const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
         if (tile >= F.ntiles) continue;
@@ -240,6 +269,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
             }
             int ntaps = 0;
+            bool flushed = false;                                 // TM: the totals in tensor memory are valid
             for (int gi = 0; gi < ngrp; ++gi) {
             const unsigned char *tbuf = tapbase + (size_t)tb * TL.bytes;
             const int4 *desc = reinterpret_cast<const int4 *>(tbuf + TL.desc);
@@ -328,10 +358,32 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 if (++buf == NBUF) { buf = 0; par ^= 1u; }
                 ntaps += d.z;
                 if (TOT && (ntaps >= 48 || e + 1 == ge1)) {
+                    if (TM) {                                     // totals += partial sums, 16 columns at a time
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) {
-                        tot01[g] = __fadd2_rn(tot01[g], acc01[g]); tot23[g] = __fadd2_rn(tot23[g], acc23[g]);
-                        acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
+                        for (int hh = 0; hh < 2; ++hh) {
+                            float v[16], old[16];
+#pragma unroll
+                            for (int g = 0; g < 4; ++g) {
+                                v[4 * g] = acc01[4 * hh + g].x; v[4 * g + 1] = acc01[4 * hh + g].y;
+                                v[4 * g + 2] = acc23[4 * hh + g].x; v[4 * g + 3] = acc23[4 * hh + g].y;
+                            }
+                            if (flushed) {
+                                tmem_ld16(taddr + 16u * hh, old);
+#pragma unroll
+                                for (int i = 0; i < 16; ++i) v[i] += old[i];
+                            }
+                            tmem_st16(taddr + 16u * hh, v);
+                        }
+                        tmem_wait_st();
+                        flushed = true;
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) { acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f); }
+                    } else {
+#pragma unroll
+                        for (int g = 0; g < 8; ++g) {
+                            tot01[g] = __fadd2_rn(tot01[g], acc01[g]); tot23[g] = __fadd2_rn(tot23[g], acc23[g]);
+                            acc01[g] = make_float2(0.f, 0.f); acc23[g] = make_float2(0.f, 0.f);
+                        }
                     }
                     ntaps = 0;
                 }
@@ -339,7 +391,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
 
             // ---- uncertain taps of this group: canonical fp64 decision per pixel pair and image -----
             if (nexc > 0) {
-                float2 *s01 = TOT ? tot01 : acc01, *s23 = TOT ? tot23 : acc23;     // the set that holds the sums so far
+                float2 *s01 = (TOT && !TM) ? tot01 : acc01, *s23 = (TOT && !TM) ? tot23 : acc23;   // a set that is in registers now
                 float tt[4][8];
 #pragma unroll
                 for (int g = 0; g < 8; ++g) { tt[0][g] = s01[g].x; tt[1][g] = s01[g].y; tt[2][g] = s23[g].x; tt[3][g] = s23[g].y; }
@@ -387,6 +439,18 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
 #pragma unroll
                 for (int g = 0; g < 8; ++g) { tot01[g] = acc01[g]; tot23[g] = acc23[g]; }
             }
+            if (TM) {                                             // totals from tensor memory + what the exact pairs added
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                    float old[16];
+                    tmem_ld16(taddr + 16u * hh, old);
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        tot01[4 * hh + g] = make_float2(old[4 * g] + acc01[4 * hh + g].x, old[4 * g + 1] + acc01[4 * hh + g].y);
+                        tot23[4 * hh + g] = make_float2(old[4 * g + 2] + acc23[4 * hh + g].x, old[4 * g + 3] + acc23[4 * hh + g].y);
+                    }
+                }
+            }
 
             // ---- store: 4 consecutive pixels per image -> one 16-byte store ------------------------
             const int start_n = P.start[r - 1], start_s = P.start[N4 - r - 1];
@@ -401,6 +465,11 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
             }
         }
     }
+    if (TM) {                                                      // all consumer warps are done with tensor memory
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        bar_named(2, NC);
+        if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(s_tmem) : "memory");
+    }
 }
 
 // host ------------------------------------------------------------------------------------------
@@ -408,12 +477,12 @@ size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_
     return (size_t)nbuf * 8 * (4 * NC + slack) * 4 + (size_t)ntb * TapLayout(pw_max, ne_max).bytes;
 }
 
-template <int NC, int SLACK, bool TOT>
+template <int NC, int SLACK, bool TOT, bool TM>
 static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io, int B, size_t smem, int nsm, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(belt_kernel<NC, SLACK, TOT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(belt_kernel<NC, SLACK, TOT, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int grid = F.ntiles < nsm ? F.ntiles : nsm;
-    belt_kernel<NC, SLACK, TOT><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
+    belt_kernel<NC, SLACK, TOT, TM><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
     return cudaGetLastError();
 }
 
@@ -421,10 +490,12 @@ static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io
 // (256 | 128, slack 256 or 512, two accumulator sets) otherwise
 cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, size_t smem, int nsm,
                         cudaStream_t st) {
-    if (threads == 512 && slack == 64) return launch_belt_nc<512, 64, false>(P, F, io, B, smem, nsm, st);
-    if (threads == 256 && slack == 256) return launch_belt_nc<256, 256, true>(P, F, io, B, smem, nsm, st);
-    if (threads == 256 && slack == 512) return launch_belt_nc<256, 512, true>(P, F, io, B, smem, nsm, st);
-    if (threads == 128 && slack == 256) return launch_belt_nc<128, 256, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 512 && slack == 64) return launch_belt_nc<512, 64, false, false>(P, F, io, B, smem, nsm, st);
+    if (threads == 512 && slack == 256) return launch_belt_nc<512, 256, true, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 512 && slack == 512) return launch_belt_nc<512, 512, true, true>(P, F, io, B, smem, nsm, st);
+    if (threads == 256 && slack == 256) return launch_belt_nc<256, 256, true, false>(P, F, io, B, smem, nsm, st);
+    if (threads == 256 && slack == 512) return launch_belt_nc<256, 512, true, false>(P, F, io, B, smem, nsm, st);
+    if (threads == 128 && slack == 256) return launch_belt_nc<128, 256, true, false>(P, F, io, B, smem, nsm, st);
     return cudaErrorInvalidValue;
 }
 

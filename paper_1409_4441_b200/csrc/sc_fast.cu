@@ -773,6 +773,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     {
         const double mean_nb_b = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
         if (N % 2048 == 0 && mean_nb_b <= 700.0 && !std::getenv("SC_BELT_NO512")) bvars.push_back({512, 64});
+        if (N % 2048 == 0 && mean_nb_b > 700.0 && !std::getenv("SC_BELT_NOTMEM")) { bvars.push_back({512, 256}); bvars.push_back({512, 512}); }
         if (N % 1024 == 0) { bvars.push_back({256, 256}); bvars.push_back({256, 512}); }
         else if (N % 512 == 0) bvars.push_back({128, 256});
     }
@@ -823,7 +824,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
                 if (bsmem + 2048 <= (size_t)smem_optin) { ntb = cb[0]; nbuf = cb[1]; break; }
             }
         }
-        if (nbuf >= (bNC == 512 ? 3 : 2)) {
+        if (nbuf >= ((bNC == 512 && bv.slack == 64) ? 3 : 2)) {
             if ((e = cudaMalloc((void **)&fp->woff, woff.size() * sizeof(int))) != cudaSuccess) return fail(e);
             if ((e = cudaMemcpy(fp->woff, woff.data(), woff.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             if ((e = cudaMalloc((void **)&fp->belt_tiles, btiles.size() * sizeof(int4))) != cudaSuccess) return fail(e);
