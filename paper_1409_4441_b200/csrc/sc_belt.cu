@@ -91,25 +91,6 @@ __device__ __forceinline__ void belt_window(const PairEnt &pe, int sh, int k0, i
 }
 
 
-// ---- tensor memory (TMEM) as accumulator storage -------------------------------------------------------------
-// 512 consumer threads leave 104 registers each: the running totals (32 floats per thread) of the
-// two-accumulator summation do not fit next to the 32 per-ring accumulators, so they live in tensor memory:
-// a warp owns the 32 TMEM lanes of its quadrant (warp % 4) and 32 columns (warp / 4); tcgen05.ld / st with the
-// 32x32b shape move one row (lane) x 16 columns per thread.
-__device__ __forceinline__ void tmem_st16(unsigned taddr, const float (&v)[16]) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                 :: "r"(taddr), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]),
-                    "f"(v[8]), "f"(v[9]), "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15]) : "memory");
-}
-__device__ __forceinline__ void tmem_ld16(unsigned taddr, float (&v)[16]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
-                   "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
-                 : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-
 // SLACK: floats per staged plane beyond the tile (window + alignment); TOT: second accumulator set
 // (flushed every >= 48 taps; needed for discs of thousands of pixels, costs 32 registers).
 // TM: the second accumulator set lives in tensor memory (512-consumer variant for large discs).

@@ -89,8 +89,8 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 // kSymBuf stage buffers; there is no block-wide barrier after the prologue.
 // TOT: per-step partial sums are added to a second accumulator set (pairwise-like summation; needed for
 // discs of thousands of pixels, costs 8 R B registers).
-// Z: two-zone table (lookup at tau(t), R11).
-template <int B, int R, int NC, bool TOT, bool Z>
+// Z: two-zone table (lookup at tau(t), R11).  TM: the second accumulator set lives in tensor memory.
+template <int B, int R, int NC, bool TOT, bool Z, bool TM>
 __global__ void __launch_bounds__(NC + kSymProd, 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(R == 1 || R == 2 || R == 4, "R");
@@ -110,7 +110,14 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
         for (int i = 0; i < kSymBuf; ++i) { mbar_init(&full_bar[i], kSymProd); mbar_init(&empty_bar[i], NC / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    __shared__ unsigned s_tmem;
+    if (TM && tid < 32) {                                  // 128 TMEM columns: warp w uses lanes 32 (w % 4) .., columns 32 (w / 4) ..
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"(smem_u32(&s_tmem)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (TM) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     unsigned it = 0;                                     // steps so far: buffer it % kSymBuf, use it / kSymBuf
     int rem_unused;
 
@@ -182,6 +189,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
     if (NC == 384) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
     const int warp = tid >> 5, lane = tid & 31;
+    const unsigned taddr = TM ? s_tmem + ((((unsigned)warp & 3u) * 32u) << 16) + ((unsigned)warp >> 2) * 32u : 0u;
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
     const float tmax = P.tmax, eps = P.eps;
     // shared-memory byte address of tab[0] minus 8 kMagicBits (mod 2^32): tab[bits - kMagicBits] = [tab_sh + 8 bits]
@@ -229,6 +237,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 #pragma unroll
                 for (int g = 0; g < 4; ++g) acc[rr][b][g] = f2(0.f);
 
+        bool flushed = false;                              // TM: the totals in tensor memory are valid
         PairEnt pe_next = F.pairs[me.e0];
         for (int step = 0; step < nsteps; ++step, ++it) {
             const int buf = it % kSymBuf;
@@ -376,7 +385,29 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     if (R == 4) { body(pos++, std::integral_constant<int, 14 & kAll>{}); body(pos++, std::integral_constant<int, 12 & kAll>{}); }
                     body(pos++, std::integral_constant<int, (1 << (R - 1))>{});
                 }
-                if (TOT) {
+                if (TOT && TM) {                                 // totals (tensor memory) += this ring's sums
+                    static_assert(!TM || (R == 4 && B == 1), "TM variant: 32 accumulators per thread");
+#pragma unroll
+                    for (int hh = 0; hh < 2; ++hh) {
+                        float v[16], old[16];
+#pragma unroll
+                        for (int q = 0; q < 2; ++q)
+#pragma unroll
+                            for (int g = 0; g < 4; ++g) {
+                                float2 &a = acc[(2 * hh + q) % R][0][g];
+                                v[8 * q + 2 * g] = a.x; v[8 * q + 2 * g + 1] = a.y;
+                                a = f2(0.f);
+                            }
+                        if (flushed) {
+                            tmem_ld16(taddr + 16u * hh, old);
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) v[i] += old[i];
+                        }
+                        tmem_st16(taddr + 16u * hh, v);
+                    }
+                    tmem_wait_st();
+                    flushed = true;
+                } else if (TOT) {
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr)
 #pragma unroll
@@ -392,6 +423,17 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             if (lane == 0) mbar_arrive(&empty_bar[buf]);         // this warp is done with the buffer
         }
 
+        if (TM && flushed) {                               // totals back from tensor memory
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                float old[16];
+                tmem_ld16(taddr + 16u * hh, old);
+#pragma unroll
+                for (int q = 0; q < 2; ++q)
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) tot[(2 * hh + q) % R][0][g] = f2(old[8 * q + 2 * g], old[8 * q + 2 * g + 1]);
+            }
+        }
         // store the 8 images of every valid base pixel
         if (active) {
             const int start_n = P.start[r - 1], start_s = P.start[4 * N - r - 1];
@@ -413,6 +455,11 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 }
             }
         }
+    }
+    if (TM) {                                              // every consumer warp is done with tensor memory
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        asm volatile("bar.sync 2, %0;" ::"r"(NC) : "memory");
+        if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(s_tmem) : "memory");
     }
 }
 
@@ -508,6 +555,7 @@ struct FastCfg {            // per batch size
     size_t smem = 0;
     SymTile *tiles = nullptr;     // [0, ntiles): all rings, work sorted; then the latitude chunks
     int ntiles = 0, ntiles_all = 0, run = 0;
+    bool tmem = false;            // 384-consumer variant with the running totals in tensor memory (large discs)
     std::map<std::pair<int, int>, std::pair<SymTile *, int>> band_tiles;   // (ring lo, hi) -> device tile list
     std::vector<int> ch_off, ch_lo, ch_hi;   // chunk i: tiles [ch_off[i], ch_off[i+1]), base rings ch_lo[i] .. ch_hi[i]
 };
@@ -533,15 +581,15 @@ struct FastPlan {
     int *grp_off = nullptr, *grp_e = nullptr;
 };
 
-template <int B, int R, int NC, bool TOT, bool Z>
+template <int B, int R, int NC, bool TOT, bool Z, bool TM = false>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st,
                               const SymTile *tiles, int nt) {
     FastDev F{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s};
-    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT, Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT, Z, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, nt);
     if (grid <= 0) return cudaSuccess;
-    sym_kernel<B, R, NC, TOT, Z><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC, TOT, Z, TM><<<grid, c.threads + kSymProd, c.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
@@ -555,7 +603,10 @@ static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev 
                                         : launch_sym<BB, RR, 256, true, false>(fp, c, P, io, st, tiles, nt))  \
                              : (P.zoned ? launch_sym<BB, RR, 128, true, true>(fp, c, P, io, st, tiles, nt)    \
                                         : launch_sym<BB, RR, 128, true, false>(fp, c, P, io, st, tiles, nt));
-    if (B == 1 && c.R == 4 && c.threads == 384) {
+    if (B == 1 && c.R == 4 && c.threads == 384 && c.tmem) {
+        e = P.zoned ? launch_sym<1, 4, 384, true, true, true>(fp, c, P, io, st, tiles, nt)
+                    : launch_sym<1, 4, 384, true, false, true>(fp, c, P, io, st, tiles, nt);
+    } else if (B == 1 && c.R == 4 && c.threads == 384) {
         e = P.zoned ? launch_sym<1, 4, 384, false, true>(fp, c, P, io, st, tiles, nt)
                     : launch_sym<1, 4, 384, false, false>(fp, c, P, io, st, tiles, nt);
     } else {
@@ -870,7 +921,9 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         // running sums, good to ~3e-7 relative rms for discs of a few hundred pixels (measured 2.7e-7 at
         // 425), so only while the mean disc holds at most 700 pixels (4.7e-7 measured at 1380 for a Gaussian, 6.9e-7 at 960 for a cancelling split kernel)
         const double mean_nb = 0.5 * (double)P.npix * ((double)P.tmax / P.scale);
-        if (B == 1 && mean_nb <= 700.0) cands = {{384, 4}, {256, 4}, {256, 2}, {128, 2}};
+        // between 700 and 6000 pixels per disc the 384-consumer variant keeps the running totals in tensor memory
+        // (4-6 % faster than 256 consumers with both sets in registers; slower again for still larger discs)
+        if (B == 1 && (mean_nb <= 700.0 || (mean_nb <= 6000.0 && !std::getenv("SC_SYM_NOTMEM")))) cands = {{384, 4}, {256, 4}, {256, 2}, {128, 2}};
         else if (B == 1) cands = {{256, 4}, {256, 2}, {128, 2}};
         else cands = {{256, 2}, {128, 2}, {128, 1}};
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
@@ -912,6 +965,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if (smem + 256 > (size_t)smem_optin) continue;        // 256: static shared memory (barriers)
             c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
             c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all; c.run = run;
+            c.tmem = (B == 1 && cd.threads == 384 && mean_nb > 700.0);      // large discs: two-level sums, totals in TMEM
             if ((e = cudaMalloc((void **)&c.tiles, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return fail(e);
             if (!tiles.empty() && (e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             c.ok = true;
