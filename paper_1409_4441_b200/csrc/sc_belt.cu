@@ -12,15 +12,15 @@
 //     bulk copies (cp.async.bulk) into a ring of NBUF buffers guarded by full/empty mbarriers;
 //   * three producer warps evaluate the taps W[r'][j] of the NEXT tile -- same fp32 geometry, table
 //     lookup and inclusion rule as the sym kernel (uncertain taps are set to 0 and decided per pixel
-//     pair in fp64 by the consumers afterwards) -- into the other of two tap buffers.
+//     pair in fp64 by the consumers afterwards) -- into the other of two tap buffers; for large discs the
+//     input rings are cut into groups and the tap buffers cycle through the groups.
+// The first / last chunk of every input ring run bodies without the FFMA2s whose taps are zero by alignment;
+// the 512-consumer large-disc variant keeps its running totals in tensor memory (tcgen05.ld/st).
 // There is no block-wide barrier after the prologue.
 #include "sc_fast.cuh"
 
 #include <type_traits>
 
-#ifndef SC_BELT_PREFETCH
-#define SC_BELT_PREFETCH 0
-#endif
 
 namespace sc {
 

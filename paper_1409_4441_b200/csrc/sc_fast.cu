@@ -5,9 +5,12 @@
 //    shared by its 8 images (4 quadrants x north/south).  A thread owns a BASE pixel (ring r <= 2N,
 //    in-ring index k < ring_length/4), evaluates the pair geometry and the table lookup once and
 //    FMA-accumulates 8 outputs (times B maps): (5 + 1 + 8 B) FMA-pipe operations per 8 B pair-maps.
-//  * A CTA owns a tile of consecutive base pixels on one ring.  For each input ring within theta_max
-//    it stages the needed run of map values -- the 4 quadrant images interleaved as float4, north and
-//    south planes -- into shared memory with cp.async, double buffered, one __syncthreads per ring.
+//  * A persistent CTA works through tiles (runs of consecutive base pixels on one ring; several short runs
+//    of the rings near the pole are packed into one tile).  It is warp-specialised: a producer warpgroup
+//    stages, for every input ring within theta_max, the needed run of map values -- the 4 quadrant images
+//    interleaved as float4, north and south planes -- into shared memory with cp.async, reporting to
+//    full/empty mbarriers; 1-3 consumer warpgroups (setmaxnreg gives them the producers' registers) run the
+//    pair loop, R adjacent base pixels per thread.  No block-wide barrier after the prologue.
 //  * Pair geometry in fp32 without cancellation: t = A + B (1 - cos d) with A, B per ring pair from
 //    fp64, d = azimuth difference built from the INTEGER pixel offset (exact) times the ring's pixel
 //    spacing; 1 - cos d by a 3-term even polynomial (|d| <= ~0.4 rad on the rings this kernel takes;
@@ -17,6 +20,8 @@
 //  * Inclusion: t < tmax - 1 needs no test at all (fast path); the last cell and everything beyond
 //    takes a branch: t > tmax + eps -> excluded, |t - tmax| <= eps -> canonical fp64 test for each
 //    of the 8 images separately (bit-exact with the oracle), else included.
+//  * Sums: per-ring partial sums added to running totals (registers, or tensor memory via tcgen05.ld/st for
+//    the 384-consumer variant on mid-size discs); a single set for discs of at most 700 pixels.
 #include "sc_fast.cuh"
 
 #include <algorithm>
