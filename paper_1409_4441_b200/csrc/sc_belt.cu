@@ -49,7 +49,8 @@ static __device__ __noinline__ unsigned belt_exact_mask(const Dev &P, int r, int
 __device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j, float dcc, bool &unc, float &Ku) {
     const float d = fmaf((float)j, pe.dphi, dcc);
     const float y = d * d;
-    float h = fmaf(y, pe.c3, pe.c2);
+    float h = fmaf(y, pe.c4, pe.c3);
+    h = fmaf(y, h, pe.c2);
     h = fmaf(y, h, pe.c1);
     const float tp = fmaf(y, h, pe.A);
     const unsigned bits = __float_as_uint(tp + kMagic);

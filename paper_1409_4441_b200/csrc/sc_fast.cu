@@ -13,7 +13,7 @@
 //    pair loop, R adjacent base pixels per thread.  No block-wide barrier after the prologue.
 //  * Pair geometry in fp32 without cancellation: t = A + B (1 - cos d) with A, B per ring pair from
 //    fp64, d = azimuth difference built from the INTEGER pixel offset (exact) times the ring's pixel
-//    spacing; 1 - cos d by a 3-term even polynomial (|d| <= ~0.4 rad on the rings this kernel takes;
+//    spacing; 1 - cos d by a 4-term even polynomial (|d| <= ~0.9 rad on the rings this kernel takes;
 //    the few rings next to the poles go to the generic kernel).
 //  * Table lookup: magic-number rounding gives the cell index; K = a_i + t b_i (one FFMA); the
 //    16K-entry (a, b) table lives in shared memory (128 KB).
@@ -295,7 +295,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     }
                 };
 
-                const float2 dphi2 = f2(pe.dphi), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
+                const float2 dphi2 = f2(pe.dphi), c4 = f2(pe.c4), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
                 // two-zone table: with t2 = t - 1/2, alpha t - 1/2 = alpha t2 + (alpha - 1)/2 and gamma (t - t1) - 1/2 = gamma t2 + gamma/2 - gamma t1 - 1/2
                 const float2 za2 = f2(P.z_alpha), zao2 = f2(0.5f * P.z_alpha - 0.5f), zg2 = f2(P.z_gamma), zgo2 = f2(0.5f * P.z_gamma - P.z_t1g - 0.5f);
                 const float zhm1f = (float)P.z_hm1;
@@ -319,7 +319,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         if (!((mask >> (2 * h)) & 3)) continue;
                         const float2 d = __ffma2_rn(jf, dphi2, dc2[h]);
                         const float2 y = __fmul2_rn(d, d);
-                        float2 p = __ffma2_rn(y, c3, c2);
+                        float2 p = __ffma2_rn(y, c4, c3);
+                        p = __ffma2_rn(y, p, c2);
                         p = __ffma2_rn(y, p, c1);
                         const float2 t2 = __ffma2_rn(y, p, A2);          // t - 0.5
                         const float2 bb = __fadd2_rn(t2, f2(kMagic));
@@ -758,8 +759,9 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         return 12 * N * N - 2 * m * (m + 1);
     };
     const double tmax = (double)(P.ntab - 1);
-    // largest |d| for which the 3-term polynomial of 1 - cos d is good to 0.004 table cells
-    const double dmax = std::min(0.45, std::pow(0.004 * 20160.0 / tmax, 1.0 / 6.0));
+    // largest |d| for which the 4-term polynomial of 1 - cos d is good to 0.004 table cells: the next term is
+    // B scale d^10 / 3628800 with B scale <= 2 tmax / d^2 for a pair inside the disc
+    const double dmax = std::min(0.9, std::pow(0.004 * 1814400.0 / tmax, 1.0 / 8.0));
 
     std::vector<PairEnt> pairs;
     std::vector<int> pair_off(1, 0);
@@ -784,7 +786,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((hw + 1 + Rmax) * dphi > dmax) ok = false;
             PairEnt e;
             e.A = (float)(A64 * P.scale - 0.5);
-            e.c1 = (float)(Bs / 2.0); e.c2 = (float)(-Bs / 24.0); e.c3 = (float)(Bs / 720.0);
+            e.c1 = (float)(Bs / 2.0); e.c2 = (float)(-Bs / 24.0); e.c3 = (float)(Bs / 720.0); e.c4 = (float)(-Bs / 40320.0); e.pad_ = 0;
             e.dphi = (float)dphi;
             e.cdc = (float)(M_PI / (4.0 * (double)ip * (double)ipq));
             e.rq = rq; e.hw = hw; e.ipq = ipq; e.shq = shof(rq);

@@ -8,13 +8,15 @@ constexpr int kMaxThreads = 512;
 constexpr float kMagic = 12582912.0f;             // 1.5 * 2^23: low mantissa bits = round(x)
 constexpr unsigned kMagicBits = 0x4B400000u;
 
-struct PairEnt {            // uniform per (base ring, input ring); 48 bytes
+struct PairEnt {            // uniform per (base ring, input ring); 56 bytes
     float A;                // A * scale - 0.5   (table coordinate shifted by half a cell)
     float c1, c2, c3;       // B * scale * {1/2, -1/24, 1/720}
     float dphi;             // azimuthal pixel spacing of the input ring
     float cdc;              // pi / (4 ip ip')
     int rq, hw, ipq, shq;   // input ring, half window (pixels), pixels per quadrant, shift flag
     int start_n, start_s;   // first pixel of the input ring and of its southern mirror
+    float c4;               // B * scale * (-1/40320): fourth term of 1 - cos d
+    int pad_;
 };
 
 // A tile of the sym kernel is a set of up to kMaxSub sub-tiles, each a run of base pixels on one ring that
