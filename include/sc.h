@@ -93,12 +93,15 @@ sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const do
  *   in_maps    HOST array of B DEVICE pointers, each to N_pix fp32 values (RING order),
  *              16-byte aligned.
  *   out_maps   HOST array of B DEVICE pointers, each to N_pix fp32 values, 16-byte aligned;
- *              must not alias any input.  Fully overwritten.
+ *              must not overlap any input or any other output (SC_ERR_INVALID_ARG).  Fully overwritten.
  *   B          >= 1.
  *   cuda_stream  a cudaStream_t (CUstream) passed as void*; NULL = the legacy default stream.
  * Map values are plain numbers: no bad-pixel sentinel is interpreted (paper silent).
  * Only kernel launches are enqueued (no allocation, no host synchronisation), so the call may be
- * captured into a CUDA graph.
+ * captured into a CUDA graph.  The plan itself is not modified apart from the launch counter read by
+ * sc_last_launch_count; a NESTED plan routes the maps through its plan-owned RING work buffers (sized at plan
+ * creation for min(max_batch, 4) maps; larger batches run in chunks of that size), so -- like every plan -- it
+ * serves one stream at a time.
  */
 sc_status sc_convolve(const sc_plan *plan, const float *const *in_maps, float *const *out_maps,
                       int B, void *cuda_stream);
@@ -136,7 +139,11 @@ sc_status sc_plan_info(const sc_plan *plan, int64_t *npix, int64_t *total_pairs,
  * p writes the number of included neighbours to count_dev[p] and, if sig_dev != NULL, the sum of
  * the neighbours' RING indices to sig_dev[p].  Both DEVICE pointers, N_pix entries (entry p refers to pixel p
  * in the plan's ordering; the signature sums RING indices also for NESTED plans; NESTED: synchronous).
- * Uses the same inclusion code as sc_convolve.  Asynchronous on cuda_stream.
+ * Runs the one-thread-per-pixel generic kernel in count mode, i.e. the inclusion code of SC_PATH_GENERIC (fp32
+ * table coordinate with a guard band, canonical fp64 test inside it).  sym_kernel and belt_kernel decide
+ * inclusion with their own fp32 form and the same fp64 test inside their guard band; THEIR sets are verified
+ * through the convolution itself (K == 1 table, small-integer maps: tests/test_gpu_parity.py
+ * test_exact_integer_sums_fast_kernels).  Asynchronous on cuda_stream.
  */
 sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uint64_t *sig_dev,
                                     void *cuda_stream);
@@ -197,6 +204,17 @@ sc_status sc_band_partition(const sc_plan *plan, int world, int rank, int *ring_
                             int64_t *out_rows, int64_t *in_rows);
 sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float *const *in_maps,
                            float *const *out_maps, int B, void *cuda_stream);
+
+/*
+ * sc_debug_fma_peak -- measurement only: the sustained FP32 FMA rate of the current device, measured with a
+ * register-only loop of independent FMA chains (packed = 0: scalar FFMA; packed = 1: FFMA2, the packed form the
+ * convolution kernels accumulate with) on 2 x 1024 threads per SM, best of 3 launches of a few ms.  bench.py uses
+ * it as the measured denominator of the roofline.
+ *   fma_per_s   HOST out: fp32 fused multiply-adds per second (an FFMA2 counts as two)
+ *   elapsed_ms  HOST out (may be NULL): duration of the best launch
+ * Synchronous on the legacy default stream; needs no plan.
+ */
+sc_status sc_debug_fma_peak(int packed, double *fma_per_s, double *elapsed_ms);
 
 /* Kernel launches enqueued by the last sc_convolve / sc_convolve_host on this plan. */
 int sc_last_launch_count(const sc_plan *plan);

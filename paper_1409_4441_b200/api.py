@@ -16,7 +16,7 @@ KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
 EXPORTS = ("sc_plan_create", "sc_plan_create_zoned", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
            "sc_band_partition", "sc_convolve_band",
            "sc_plan_destroy", "sc_plan_set_path",
-           "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_last_launch_count",
+           "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_debug_fma_peak", "sc_last_launch_count",
            "sc_status_string", "sc_last_cuda_error", "sc_version")
 
 _lib = None
@@ -54,6 +54,7 @@ def lib():
         l.sc_debug_neighbour_counts.argtypes = [vp, vp, vp, vp]
         l.sc_debug_stats.argtypes = [vp, vp, vp, vp]
         l.sc_last_launch_count.argtypes = [vp]
+        l.sc_debug_fma_peak.argtypes = [i32, vp, vp]
         for f in ("sc_status_string", "sc_last_cuda_error", "sc_version"):
             getattr(l, f).restype = C.c_char_p
         l.sc_status_string.argtypes = [i32]
@@ -165,6 +166,13 @@ def sc_debug_stats(plan):
 def sc_debug_neighbour_counts(plan, count_ptr, sig_ptr=0, stream=0):
     _chk(lib().sc_debug_neighbour_counts(plan, C.c_void_p(int(count_ptr)), C.c_void_p(int(sig_ptr) or None),
                                          C.c_void_p(int(stream) or None)), "sc_debug_neighbour_counts")
+
+
+def sc_debug_fma_peak(packed=True):
+    """Measurement only: sustained FP32 FMA/s of the current device (FFMA2 loop if packed else scalar FFMA)."""
+    v, ms = C.c_double(0), C.c_double(0)
+    _chk(lib().sc_debug_fma_peak(1 if packed else 0, C.byref(v), C.byref(ms)), "sc_debug_fma_peak")
+    return dict(fma_per_s=v.value, elapsed_ms=ms.value)
 
 
 def sc_last_launch_count(plan):

@@ -461,7 +461,8 @@ size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_
 
 template <int NC, int SLACK, bool TOT, bool TM>
 static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io, int B, size_t smem, int nsm, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(belt_kernel<NC, SLACK, TOT, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static bool attr_done[64] = {};
+    cudaError_t e = ensure_max_smem(belt_kernel<NC, SLACK, TOT, TM>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = F.ntiles < nsm ? F.ntiles : nsm;
     belt_kernel<NC, SLACK, TOT, TM><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);

@@ -591,7 +591,8 @@ template <int B, int R, int NC, bool TOT, bool Z, bool TM = false>
 static cudaError_t launch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, cudaStream_t st,
                               const SymTile *tiles, int nt) {
     FastDev F{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s};
-    cudaError_t e = cudaFuncSetAttribute(sym_kernel<B, R, NC, TOT, Z, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+    static bool attr_done[64] = {};
+    cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = std::min(fp->nsm, nt);
     if (grid <= 0) return cudaSuccess;

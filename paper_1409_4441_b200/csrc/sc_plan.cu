@@ -102,8 +102,8 @@ struct sc_plan {
     int polar_rings = 0;                       // rings 1..polar_rings and their southern mirrors use the generic kernel
     // NESTED plans: the kernels run on plan-owned RING buffers (nest_maps maps in, nest_maps maps out)
     int nested = 0;
-    mutable float *nest_in = nullptr, *nest_out = nullptr;
-    mutable int nest_maps = 0;
+    float *nest_in = nullptr, *nest_out = nullptr;
+    int nest_maps = 0;                         // min(max_batch, maps per launch): larger batches run in chunks of this size
 };
 
 namespace {
@@ -161,10 +161,10 @@ sc_status run_audit(sc_plan *pl) {
         if (!cuda_ok(launch_generic_count(pl->dev, nullptr, nullptr, &au, 0), "audit launch")) { st = SC_ERR_CUDA; break; }
         if (!cuda_ok(cudaDeviceSynchronize(), "audit sync")) { st = SC_ERR_CUDA; break; }
         unsigned long long tot = 0, unc = 0; unsigned int errb = 0, n = 0;
-        cudaMemcpy(&tot, d_tot, 8, cudaMemcpyDeviceToHost);
-        cudaMemcpy(&unc, d_unc, 8, cudaMemcpyDeviceToHost);
-        cudaMemcpy(&errb, d_err, 4, cudaMemcpyDeviceToHost);
-        if (!cuda_ok(cudaMemcpy(&n, d_cnt, 4, cudaMemcpyDeviceToHost), "memcpy")) { st = SC_ERR_CUDA; break; }
+        if (!cuda_ok(cudaMemcpy(&tot, d_tot, 8, cudaMemcpyDeviceToHost), "memcpy") ||
+            !cuda_ok(cudaMemcpy(&unc, d_unc, 8, cudaMemcpyDeviceToHost), "memcpy") ||
+            !cuda_ok(cudaMemcpy(&errb, d_err, 4, cudaMemcpyDeviceToHost), "memcpy") ||
+            !cuda_ok(cudaMemcpy(&n, d_cnt, 4, cudaMemcpyDeviceToHost), "memcpy")) { st = SC_ERR_CUDA; break; }
         if (n > cap) { st = SC_ERR_UNSUPPORTED; break; }   // too many knife-edge pairs to list
         float errf; std::memcpy(&errf, &errb, 4);
         pl->n_uncertain = (int64_t)unc;
@@ -379,30 +379,39 @@ sc_status sc_debug_stats(const sc_plan *plan, int64_t *n_uncertain, double *max_
 
 int sc_last_launch_count(const sc_plan *plan) { return plan ? plan->last_launches : 0; }
 
+// Maps are N_pix floats each: no output may overlap an input or another output.
+static bool maps_ok(const float *const *in_maps, float *const *out_maps, int B, size_t npix) {
+    const uintptr_t bytes = (uintptr_t)npix * 4;
+    auto overlap = [&](const void *a, const void *b) {
+        const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+        return x < y + bytes && y < x + bytes;
+    };
+    for (int b = 0; b < B; ++b) {
+        if (!in_maps[b] || !out_maps[b]) return false;
+        if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return false;
+    }
+    for (int b = 0; b < B; ++b) {
+        for (int a = 0; a < B; ++a) {
+            if (overlap(out_maps[b], in_maps[a])) return false;
+            if (a != b && overlap(out_maps[b], out_maps[a])) return false;
+        }
+    }
+    return true;
+}
+
 // ev (optional): 4 events recorded before the polar kernel and after each of the three kernels
 static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps, float *const *out_maps, int B,
                                void *cuda_stream, cudaEvent_t *ev, float *ms) {
     if (!plan || !in_maps || !out_maps || B < 1) return SC_ERR_INVALID_ARG;
-    for (int b = 0; b < B; ++b) {
-        if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
-        if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return SC_ERR_INVALID_ARG;
-        for (int a = 0; a < B; ++a) if ((const float *)out_maps[b] == in_maps[a]) return SC_ERR_INVALID_ARG;
-    }
+    if (!maps_ok(in_maps, out_maps, B, (size_t)plan->dev.npix)) return SC_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const sc::Dev &D = plan->dev;
     int launches = 0;
     const size_t npix = (size_t)D.npix;
-    if (plan->nested && plan->nest_maps < std::min(B, sc::kMaxB)) {       // RING work buffers (first use: synchronous)
-        if (plan->nest_in) cudaFree(plan->nest_in);
-        if (plan->nest_out) cudaFree(plan->nest_out);
-        plan->nest_in = plan->nest_out = nullptr; plan->nest_maps = 0;
-        const int nm = std::min(std::max(B, plan->max_batch), sc::kMaxB);
-        if (!cuda_ok(cudaMalloc((void **)&plan->nest_in, npix * 4 * nm), "cudaMalloc")) return SC_ERR_ALLOC;
-        if (!cuda_ok(cudaMalloc((void **)&plan->nest_out, npix * 4 * nm), "cudaMalloc")) return SC_ERR_ALLOC;
-        plan->nest_maps = nm;
-    }
-    for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
-        const int nb = std::min(sc::kMaxB, B - b0);
+    // maps per launch; a NESTED plan goes through its RING work buffers, which hold nest_maps maps
+    const int chunk = plan->nested ? plan->nest_maps : sc::kMaxB;
+    for (int b0 = 0; b0 < B; b0 += chunk) {
+        const int nb = std::min(chunk, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
         if (plan->nested) {                                                // NESTED -> RING work buffers
@@ -650,11 +659,7 @@ sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float 
     const int N = D.nside;
     if (ring_lo < 1 || ring_hi < ring_lo || ring_hi > 2 * N) return SC_ERR_INVALID_ARG;
     if (plan->nested) return SC_ERR_UNSUPPORTED;                       // bands are contiguous rows in RING order only
-    for (int b = 0; b < B; ++b) {
-        if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
-        if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return SC_ERR_INVALID_ARG;
-        for (int a = 0; a < B; ++a) if ((const float *)out_maps[b] == in_maps[a]) return SC_ERR_INVALID_ARG;
-    }
+    if (!maps_ok(in_maps, out_maps, B, (size_t)D.npix)) return SC_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int64_t orow[4];
     band_rows(plan, ring_lo, ring_hi, orow, nullptr);

@@ -1,0 +1,70 @@
+// sc_probe.cu -- measurement only: the sustained FP32 FMA rate of the device, the denominator of the roofline
+// that bench.py reports ("report against (i) the nominal figure and (ii) a sustained FFMA
+// microbenchmark run in the same job").  Register-only loops of independent FMA chains: scalar FFMA or packed
+// FFMA2 (fma.rn.f32x2, the instruction the convolution kernels accumulate with).
+#include "../../include/sc.h"
+#include <cuda_runtime.h>
+
+namespace {
+
+constexpr int kChains = 16;          // independent fp32 accumulators per thread (8 float2 in the packed loop)
+
+template <bool PACKED>
+__global__ void __launch_bounds__(1024, 1)
+fma_probe_kernel(float *out, int iters, float a, float b) {
+    float2 acc[kChains / 2];
+#pragma unroll
+    for (int j = 0; j < kChains / 2; ++j) acc[j] = make_float2((float)threadIdx.x + j, (float)j - 0.5f);
+    const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+            for (int j = 0; j < kChains / 2; ++j) {
+                if (PACKED) acc[j] = __ffma2_rn(acc[j], a2, b2);
+                else { acc[j].x = fmaf(acc[j].x, a, b); acc[j].y = fmaf(acc[j].y, a, b); }
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < kChains / 2; ++j) s += acc[j].x + acc[j].y;
+    if (s == 123.456f) out[0] = s;       // never true in practice: keeps the loop alive
+}
+
+}  // namespace
+
+extern "C" sc_status sc_debug_fma_peak(int packed, double *fma_per_s, double *elapsed_ms) {
+    if (!fma_per_s) return SC_ERR_INVALID_ARG;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return SC_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) return SC_ERR_CUDA;
+    float *d = nullptr;
+    if (cudaMalloc((void **)&d, 4) != cudaSuccess) return SC_ERR_ALLOC;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    sc_status st = SC_OK;
+    double best = 0.0, best_ms = 0.0;
+    do {
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { st = SC_ERR_CUDA; break; }
+        const int blocks = 2 * nsm, threads = 1024, iters = 12000;       // ~ 6 ms at 128 FMA / clk / SM
+        const double fmas = (double)blocks * threads * (double)iters * 4.0 * kChains;
+        for (int rep = 0; rep < 4 && st == SC_OK; ++rep) {               // first repetition = warm-up
+            cudaEventRecord(e0, 0);
+            if (packed) fma_probe_kernel<true><<<blocks, threads>>>(d, iters, 1.000001f, 1e-7f);
+            else fma_probe_kernel<false><<<blocks, threads>>>(d, iters, 1.000001f, 1e-7f);
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { st = SC_ERR_CUDA; break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms > 0.f && fmas / (ms * 1e-3) > best) { best = fmas / (ms * 1e-3); best_ms = ms; }
+        }
+    } while (0);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(d);
+    if (st != SC_OK) return st;
+    *fma_per_s = best;
+    if (elapsed_ms) *elapsed_ms = best_ms;
+    return SC_OK;
+}

@@ -114,22 +114,42 @@ def halo_plan(bands, rank):
     return sends, recvs
 
 
+def _global_rank(group, r):
+    """Rank r of `group` as a global rank (P2POp / broadcast take global ranks)."""
+    import torch.distributed as dist
+    return r if group is None else dist.get_global_rank(group, r)
+
+
 def exchange_halos(maps, bands, rank, group=None):
     """Fill the overlap rows of the full-size tensors `maps` (valid in this rank's out_rows) from their
-    owners.  Point-to-point, one message per (peer, range, map); bytes = the overlap only."""
+    owners.  Point to point, ONE packed message per peer and direction (all ranges of all maps, in the order
+    maps outer / halo_plan ranges inner, which both sides derive identically); bytes = the overlap only.
+    `rank` and the band index are ranks within `group`.  Returns the number of elements received."""
+    import torch
     import torch.distributed as dist
     sends, recvs = halo_plan(bands, rank)
-    ops, keep = [], []
-    for m in maps:
-        for peer, lo, hi in recvs:
-            ops.append(dist.P2POp(dist.irecv, m[lo:hi], peer, group))
-        for peer, lo, hi in sends:
-            buf = m[lo:hi].contiguous()
-            keep.append(buf)
-            ops.append(dist.P2POp(dist.isend, buf, peer, group))
-    if ops:
-        for req in dist.batch_isend_irecv(ops):
-            req.wait()
+    if not sends and not recvs:
+        return 0
+    ops, unpack = [], []
+    for peer in sorted({p for p, _, _ in recvs}):
+        rng = [(lo, hi) for p, lo, hi in recvs if p == peer]
+        buf = torch.empty(sum(hi - lo for lo, hi in rng) * len(maps), dtype=maps[0].dtype, device=maps[0].device)
+        unpack.append((buf, rng))
+        ops.append(dist.P2POp(dist.irecv, buf, _global_rank(group, peer), group))
+    keep = []
+    for peer in sorted({p for p, _, _ in sends}):
+        rng = [(lo, hi) for p, lo, hi in sends if p == peer]
+        buf = torch.cat([m[lo:hi] for m in maps for lo, hi in rng])
+        keep.append(buf)
+        ops.append(dist.P2POp(dist.isend, buf, _global_rank(group, peer), group))
+    for req in dist.batch_isend_irecv(ops):
+        req.wait()
+    for buf, rng in unpack:
+        off = 0
+        for m in maps:
+            for lo, hi in rng:
+                m[lo:hi] = buf[off:off + hi - lo]
+                off += hi - lo
     return sum(hi - lo for _, lo, hi in recvs) * len(maps)
 
 
@@ -139,7 +159,7 @@ def gather_bands(maps, bands, group=None):
     for m in maps:
         for owner, b in enumerate(bands):
             for lo, hi in _ranges(b["out_rows"]):
-                dist.broadcast(m[lo:hi], src=owner, group=group)
+                dist.broadcast(m[lo:hi], src=_global_rank(group, owner), group=group)
 
 
 def convolve_banded(plan, maps_in, maps_out, group=None, gather=False):

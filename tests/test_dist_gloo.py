@@ -179,3 +179,55 @@ def test_halo_plan_is_consistent():
             assert (r, lo, hi) in D.halo_plan(bands, peer)[1]
     assert D._subtract([(0, 10)], [(2, 4), (6, 20)]) == [(0, 2), (4, 6)]
     assert D._intersect([(0, 10), (20, 30)], [(5, 25)]) == [(5, 10), (20, 25)]
+
+
+def _subgroup_worker(rank, world, port, q):
+    """Ranks 0 and 2 of a 3-rank job form a group and share TWO maps in two latitude bands: exercises the mapping of
+    group ranks to global ranks in exchange_halos / gather_bands and the packed one-message-per-peer layout."""
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+    from paper_1409_4441_b200 import dist as D
+    from workloads import gen
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        grp = dist.new_group([0, 2])
+        if rank in (0, 2):
+            nside, theta = 8, 20.0 * gen.DEG
+            npix = 12 * nside * nside
+            grank = dist.get_rank(grp)
+            bands = _cpu_bands(nside, theta, 2)
+            full = [gen.noise_map(npix, 77), gen.noise_map(npix, 78)]
+            local = []
+            for f in full:
+                t = torch.full((npix,), float("nan"), dtype=torch.float32)
+                for lo, hi in D._ranges(bands[grank]["out_rows"]):
+                    t[lo:hi] = torch.from_numpy(f[lo:hi])
+                local.append(t)
+            D.exchange_halos(local, bands, grank, grp)
+            ok = True
+            for t, f in zip(local, full):
+                for lo, hi in D._ranges(bands[grank]["in_rows"]):
+                    ok = ok and bool(np.array_equal(t[lo:hi].numpy(), f[lo:hi]))
+            D.gather_bands(local, bands, grp)           # own rows are valid everywhere -> complete maps on both ranks
+            ok = ok and all(np.array_equal(t.numpy(), f) for t, f in zip(local, full))
+            q.put((rank, ok))
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_halo_exchange_in_a_subgroup_with_two_maps():
+    world = 3
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_subgroup_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    results = [q.get(timeout=240) for _ in range(2)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert sorted(r for r, _ in results) == [0, 2] and all(ok for _, ok in results)

@@ -105,17 +105,38 @@ def test_config2_full_batch2(sc, path):
             _check_values(out[b], ref[b], f"cfg2/{path}/map{b}")
 
 
-def _sampled_config(sc, ci, key, n_val, n_cnt, path="auto"):
+def _ring_pixels(tb, rings):
+    return np.concatenate([np.arange(tb["start"][r - 1], tb["start"][r - 1] + tb["npr"][r - 1]) for r in rings])
+
+
+def _structured_subset(nside, theta_max):
+    """SURVEY.md 8d's deterministic subset for maps too large for a full oracle pass: every 16th ring plus all rings
+    within theta_max of the poles and of the cap/belt boundary rings N and 3N (whole rings, so tile boundaries and
+    ragged tails are inside), plus the equator ring."""
+    tb = O.ring_table(nside)
+    th = np.arccos(np.clip(tb["z"], -1.0, 1.0))
+    N = nside
+    near = lambda t0: np.abs(th - t0) <= theta_max * 1.02
+    keep = near(0.0) | near(np.pi) | near(th[N - 1]) | near(th[3 * N - 1])
+    keep[15::16] = True
+    keep[2 * N - 1] = True
+    rings = np.nonzero(keep)[0] + 1
+    return _ring_pixels(tb, rings), rings
+
+
+def _config_parity(sc, ci, key, sel=None, n_cnt=200000):
+    """Values (all maps of the batch) and neighbour sets against the oracle: on every pixel (sel None) or on `sel`;
+    the exact pair total over the sphere and counts + signatures on n_cnt further sampled pixels in both cases."""
     cfg = gen.config(ci)
     T, maps = gen.table_for(cfg), gen.maps_for(cfg)
-    sel_v = gen.sample_pixels(cfg.nside, n_val, seed=100 + ci)
+    ref, cnt_v, sig_v = O.convolve(cfg.nside, T, cfg.theta_max, maps, sel=sel)
+    pix = np.arange(cfg.npix) if sel is None else sel
+    print(f"cfg{ci}: oracle on {pix.size} of {cfg.npix} pixels ({100.0 * pix.size / cfg.npix:.1f} %), {O.last_threads()} threads")
     sel_c = gen.sample_pixels(cfg.nside, n_cnt, seed=200 + ci)
-    ref, cnt_v, sig_v = O.convolve(cfg.nside, T, cfg.theta_max, maps, sel=sel_v)
     cnt_c, sig_c = O.count(cfg.nside, cfg.theta_max, sel=sel_c)
     with sc.Plan(cfg.nside, T, cfg.theta_max, cfg.batch) as plan:
-        _set_path(sc, plan, path)
         info = plan.info()
-        print("audit:", info)
+        print("audit:", info, plan.partition())
         assert info["total_pairs"] == _totals()[key]
         assert info["max_t_err"] < info["guard_band"]
         cnt, sig = plan.neighbour_counts()
@@ -123,30 +144,37 @@ def _sampled_config(sc, ci, key, n_val, n_cnt, path="auto"):
         assert int(cnt.astype(np.int64).sum()) == _totals()[key]
         np.testing.assert_array_equal(cnt[sel_c], cnt_c)
         np.testing.assert_array_equal(sig[sel_c], sig_c)
-        np.testing.assert_array_equal(cnt[sel_v], cnt_v)
-        np.testing.assert_array_equal(sig[sel_v], sig_v)
+        np.testing.assert_array_equal(cnt[pix], cnt_v)
+        np.testing.assert_array_equal(sig[pix], sig_v)
         out = _gpu_convolve(sc, plan, maps)
         for b in range(cfg.batch):
-            # normalise by the statistics of the sampled reference (white-noise map: stationary)
-            _check_values(out[b][sel_v], ref[b], f"cfg{ci}/{path}/map{b}")
+            _check_values(out[b][pix], ref[b], f"cfg{ci}/map{b}")
             assert np.all(np.isfinite(out[b]))
-        return out
+        return out, ref, pix
 
 
-def test_config3_sampled(sc):
-    """Nside 1024, theta_max 30': exact pair total over the sphere; counts on 200k and values on 20k
-    sampled pixels (poles, cap/belt boundaries, equator + seeded random)."""
-    _sampled_config(sc, 3, (1024, 30), 20000, 200000)
+def test_config3_full_map(sc):
+    """Nside 1024, theta_max 30': EVERY pixel against the oracle (values, counts, signatures), exact pair total."""
+    _config_parity(sc, 3, (1024, 30))
 
 
-def test_config4_sampled(sc):
-    """Nside 2048, theta_max 20', split-like oscillating kernel (the metric's configuration)."""
-    _sampled_config(sc, 4, (2048, 20), 20000, 200000)
+def test_config4_full_map(sc):
+    """Nside 2048, theta_max 20', split-like oscillating kernel (the metric's configuration): EVERY pixel of the
+    50,331,648 against the oracle (the full oracle pass takes well under 10 min on the box)."""
+    out, ref, _ = _config_parity(sc, 4, (2048, 20))
+    # per ring as well, so that one broken short ring or tile cannot hide in the all-sky average
+    tb = O.ring_table(2048)
+    err2 = np.add.reduceat((out[0].astype(np.float64) - ref[0]) ** 2, tb["start"]) / tb["npr"]
+    assert np.sqrt(err2.max() / np.mean(ref[0] ** 2)) <= 2 * REL_RMS_TOL, int(np.argmax(err2)) + 1
 
 
-def test_config5_sampled_batch3(sc):
-    """Nside 2048, theta_max 60', B = 3."""
-    _sampled_config(sc, 5, (2048, 60), 4000, 50000)
+def test_config5_structured_subset_batch3(sc):
+    """Nside 2048, theta_max 60', B = 3: SURVEY.md 8d's structured subset (every 16th ring + all rings within theta_max
+    of the poles and of rings N, 3N + the equator, whole rings: >= 5 % of the pixels), all three maps."""
+    cfg = gen.config(5)
+    sel, rings = _structured_subset(cfg.nside, cfg.theta_max)
+    assert sel.size >= 0.05 * cfg.npix
+    _config_parity(sc, 5, (2048, 60), sel=sel, n_cnt=50000)
 
 
 def test_config6_paper_scale_sampled(sc):
@@ -214,6 +242,51 @@ def test_exact_integer_sums(sc, path):
             _set_path(sc, plan, path)
             out = _gpu_convolve(sc, plan, [m])
         np.testing.assert_array_equal(out[0], want)
+
+
+def _handover_rings(N, pr, fb):
+    """Whole rings at every kernel hand-over of the AUTO path (polar | sym | belt) and at the cap/belt boundary and the
+    equator, with their southern mirrors."""
+    fbm = min(fb, 2 * N)
+    base = {1, 2, pr, pr + 1, fbm - 1, fbm, N - 1, N, N + 1, 2 * N - 1, 2 * N}
+    base = {r for r in base if 1 <= r <= 2 * N}
+    return sorted(base | {4 * N - r for r in base} | {2 * N + 1})
+
+
+@pytest.mark.parametrize("nside,theta_am,ntab,B", [
+    (512, 60, 4096, 1),        # belt_kernel<128>, sym 384-consumer variant
+    (1024, 30, 8192, 1),       # config 3's launch configuration: belt_kernel<256>
+    (1024, 72, 8192, 1),       # discs of ~1500 pixels: running totals in tensor memory (sym), two sets (belt<256>)
+    (2048, 20, 16384, 1),      # config 4's launch configuration: belt_kernel<512, 64>, single accumulator set
+    (2048, 60, 16384, 1),      # belt_kernel<512, 256, TM>, sym TMEM variant
+    (2048, 60, 16384, 3)])     # config 5's launch configuration (B = 3)
+def test_exact_integer_sums_fast_kernels(sc, nside, theta_am, ntab, B):
+    """north_star: "GPU neighbour enumeration must be bit-exact" -- measured on the kernels that do the work.  K == 1
+    table of the config's size and small-integer maps through SC_PATH_AUTO at the sizes that select every variant of
+    sym_kernel / belt_kernel / generic_warp_kernel: every product and sum is exact in fp32, so out == fl32(sum) * fl32(Omega)
+    bit for bit iff the neighbour SET those kernels used is the oracle's.  Oracle on whole rings at every kernel hand-over
+    plus 20,000 random pixels."""
+    theta = theta_am * gen.ARCMIN
+    npix = 12 * nside * nside
+    T = np.ones(ntab)
+    maps = [np.random.default_rng(100 * nside + theta_am + b).integers(-8, 9, size=npix).astype(np.float32) for b in range(B)]
+    tb = O.ring_table(nside)
+    with sc.Plan(nside, T, theta, B) as plan:
+        part = plan.partition()
+        assert part["polar_rings"] < part["first_belt_ring"] <= 2 * nside, part      # all three kernels are in use
+        rings = _handover_rings(nside, part["polar_rings"], part["first_belt_ring"])
+        sel = np.unique(np.concatenate([_ring_pixels(tb, rings), gen.sample_pixels(nside, 20000, seed=nside + theta_am)]))
+        out = _gpu_convolve(sc, plan, maps)
+        assert sc.sc_last_launch_count(plan.handle) == 3
+    ref, cnt, _ = O.convolve(nside, T, theta, maps, sel=sel)
+    omega64 = 4 * np.pi / npix
+    omega = np.float32(omega64)
+    for b in range(B):
+        s = np.rint(ref[b] / omega64)
+        assert np.max(np.abs(ref[b] / omega64 - s)) < 1e-6 and np.max(np.abs(s)) < 2 ** 24
+        want = s.astype(np.float32) * omega
+        bad = np.nonzero(out[b][sel] != want)[0]
+        assert bad.size == 0, (part, sel[bad[:10]], out[b][sel][bad[:10]], want[bad[:10]])
 
 
 @pytest.mark.parametrize("path", PATHS)
@@ -352,6 +425,49 @@ def test_latitude_bands(sc, ci, world):
             plan.band(0, 0)
         with pytest.raises(sc.ScError):
             sc.sc_convolve_band(plan.handle, 5, 4, [m.data_ptr()], [out.data_ptr()])
+
+
+@pytest.mark.parametrize("ci,world,B", [(1, 2, 1), (2, 3, 2), (3, 4, 1), (3, 8, 1)])
+def test_bands_with_simulated_halo_exchange(sc, ci, world, B):
+    """The PRODUCT's sc_band_partition output driven through dist.halo_plan with `world` simulated ranks on one GPU:
+    every rank has a full-size buffer that is valid in its own rows only (NaN elsewhere), the copies halo_plan prescribes
+    are carried out between the buffers, every rank convolves its band, and the union equals sc_convolve bit for bit.
+    (The gloo tests exercise the same halo_plan with real point-to-point messages; this one ties it to the kernels.)"""
+    import torch
+    from paper_1409_4441_b200 import dist as D
+    cfg = gen.config(ci)
+    T = gen.table_for(cfg)
+    maps = [torch.from_numpy(gen.noise_map(cfg.npix, 600 + 7 * ci + b)).cuda() for b in range(B)]
+    with sc.Plan(cfg.nside, T, cfg.theta_max, B) as plan:
+        full = plan.convolve(maps)
+        bands = [plan.band(world, r) for r in range(world)]
+        own = [D._ranges(b["out_rows"]) for b in bands]
+        bufs = []
+        for r in range(world):
+            mine = [torch.full_like(m, float("nan")) for m in maps]
+            for t, m in zip(mine, maps):
+                for lo, hi in own[r]:
+                    t[lo:hi] = m[lo:hi]
+            bufs.append(mine)
+        plans = [D.halo_plan(bands, r) for r in range(world)]
+        for r in range(world):
+            sends, recvs = plans[r]
+            for peer, lo, hi in sends:                          # both sides agree on every message
+                assert (r, lo, hi) in plans[peer][1]
+            for peer, lo, hi in recvs:
+                assert (r, lo, hi) in plans[peer][0]
+                assert any(a <= lo and hi <= b for a, b in own[peer])      # the sender owns what it sends
+                for t, src in zip(bufs[r], bufs[peer]):
+                    t[lo:hi] = src[lo:hi]
+        out = [torch.full_like(m, float("nan")) for m in maps]
+        for r in range(world):
+            for t in bufs[r]:                                   # everything the band reads has arrived
+                for lo, hi in D._ranges(bands[r]["in_rows"]):
+                    assert not bool(torch.isnan(t[lo:hi]).any())
+            plan.convolve_band(bands[r]["ring_lo"], bands[r]["ring_hi"], bufs[r], out)
+        torch.cuda.synchronize()
+        for o, f in zip(out, full):
+            assert torch.equal(o, f)
 
 
 def test_profile_entry_and_partition(sc):
