@@ -42,6 +42,19 @@ struct FastDev {
     int ntab_s;             // entries of the shared-memory table
 };
 
+// What a launch of the sym kernel needs from the plan (host); the instantiations live in sc_sym_b1.cu (one map per
+// launch: 8 images, 16 images with the mirror symmetry, north-only) and sc_sym_bn.cu (batches of 2-4 maps)
+struct SymLaunch {
+    const PairEnt *pairs;
+    const SymTile *tiles;
+    int ntiles, Ltot, ntab_s, nsm;
+    int threads, R;             // consumer threads, base pixels per thread
+    size_t smem;
+    bool tot, tmem, mirror, south;
+};
+cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
+cudaError_t dispatch_sym_bn(const SymLaunch &L, const Dev &P, const Maps &io, int B, cudaStream_t st);
+
 constexpr int kMaxExc = 32;      // uncertain taps per belt tile that can be listed (more -> rescan)
 
 struct BeltDev {
@@ -79,8 +92,11 @@ template <class K> inline cudaError_t ensure_max_smem(K kernel, bool (&done)[64]
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
     int optin = 0;
+    cudaFuncAttributes fa{};
     if ((e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin)) != cudaSuccess) return e;
+    if ((e = cudaFuncGetAttributes(&fa, kernel)) != cudaSuccess) return e;
+    // the opt-in limit covers static + dynamic shared memory
+    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes)) != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) done[dev] = true;
     return cudaSuccess;
 }

@@ -1,0 +1,524 @@
+// sc_sym.cuh -- the sym kernel (polar caps and the cap/belt transition) and its launcher template.
+// Included by the translation units that instantiate it (sc_sym_b1.cu: one map per launch; sc_sym_bn.cu: batches).
+//
+// Design:
+//  * HEALPix RING is invariant under phi -> phi + pi/2, z -> -z and the reflection phi -> pi/2 - phi, so the
+//    weight K(p, q) of a pair is shared by up to 16 image pairs (4 rotations x north/south x mirror).  A thread
+//    owns R adjacent BASE pixels (ring r <= 2N; in-ring index k in the first quadrant, or in its first half when
+//    the mirror images are used), evaluates the pair geometry and the table lookup once per (base pixel, input
+//    pixel) and FMA-accumulates one output per image and map with packed FFMA2.
+//    Template flags: SOUTH = z -> -z images, MIRROR = reflected images; staged planes per position
+//    NPL = (1 + SOUTH)(1 + MIRROR), each plane holding the 4 rotation images as one float4.
+//  * A persistent CTA works through tiles (runs of consecutive base pixels on one ring; several short runs
+//    of the rings near the pole are packed into one tile).  It is warp-specialised: producer warps stage, for every
+//    input ring within theta_max, the needed run of map values of every image into shared memory with 4-byte
+//    cp.async (the image runs are 4-byte-misaligned against each other, and the mirrored runs are reversed, which
+//    rules out TMA), reporting to full/empty mbarriers; the consumer warps (setmaxnreg gives them the producers'
+//    registers) run the pair loop.  No block-wide barrier after the prologue.
+//  * Pair geometry in fp32 without cancellation: t = A + B (1 - cos d) with A, B per ring pair from
+//    fp64, d = azimuth difference built from the INTEGER pixel offset (exact) times the ring's pixel
+//    spacing; 1 - cos d by a 4-term even polynomial (|d| <= ~0.9 rad on the rings this kernel takes;
+//    the few rings next to the poles go to the generic kernel).  The mirrored pair has d' = -d: same t.
+//  * Table lookup: magic-number rounding gives the cell index; K = a_i + t b_i (one FFMA); the
+//    16K-entry (a, b) table lives in shared memory (128 KB).
+//  * Inclusion: t < tmax - 1 needs no test at all (fast path); the last cell and everything beyond
+//    takes a branch: t > tmax + eps -> excluded, |t - tmax| <= eps -> canonical fp64 test for each
+//    of the images separately (bit-exact with the oracle), else included.
+//  * Sums: per-ring partial sums added to running totals (registers, or tensor memory via tcgen05.ld/st for
+//    the 384-consumer variant on mid-size discs); a single set for discs of at most 700 pixels.
+#pragma once
+#include "sc_fast.cuh"
+
+#include <algorithm>
+#include <type_traits>
+
+namespace sc {
+
+// floor(Y / d) and remainder for 0 <= Y < 2^31 with M0 = floor((2^32 - 1) / d): one multiply-high
+// and one fix-up instead of an integer division
+__device__ __forceinline__ int div_fast(int Y, int d, unsigned M0, int &rem) {
+    int q = (int)__umulhi((unsigned)Y, M0);
+    rem = Y - q * d;
+    if (rem >= d) { ++q; rem -= d; }
+    return q;
+}
+
+// Exact decisions for the images of one uncertain pair: bit 4 pl + m set <=> rotation m of plane pl included;
+// planes are ordered north, south (if `south`), north mirrored, south mirrored (if `mirror`).
+// (k, sh) / (kq, shq): in-ring index and shift flag of the base pixel / the input pixel.
+static __device__ __noinline__ unsigned sym_exact_mask(const Dev &P, int r, int k, int ip, int sh, int rq, int kq,
+                                                       int ipq, int shq, float t, int south, int mirror) {
+    const int N4 = 4 * P.nside;
+    const int n = 4 * ip, nq = 4 * ipq;
+    unsigned mask = 0;
+    kq %= nq; if (kq < 0) kq += nq;
+    int pl = 0;
+    for (int mi = 0; mi <= mirror; ++mi) {
+        // reflection phi -> pi/2 - phi: (2 k' + 1 - sh) = 2 ip - (2 k + 1 - sh)
+        int kb = mi ? ip - 1 + sh - k : k;
+        int kqb = mi ? ipq - 1 + shq - kq : kq;
+        if (kb < 0) kb += n;
+        if (kqb < 0) kqb += nq;
+        for (int h = 0; h <= south; ++h, ++pl) {
+            const int rp_i = h ? N4 - r : r, rq_i = h ? N4 - rq : rq;
+            for (int m = 0; m < 4; ++m) {
+                int kp_i = kb + m * ip; if (kp_i >= n) kp_i -= n;
+                int kq_i = kqb + m * ipq; if (kq_i >= nq) kq_i -= nq;
+                if (exact_included(P, rp_i, kp_i, rq_i, kq_i, t, nullptr)) mask |= 1u << (4 * pl + m);
+            }
+        }
+    }
+    return mask;
+}
+
+// Shared-memory slot (16-byte unit) of staged position i.  A thread owns R adjacent base pixels, so the
+// 8 lanes of a quarter warp (one LDS.128 wavefront) read positions R apart.  XOR-ing the low bits with the
+// index of the 8-position block spreads such a stride over all 8 bank groups for every alignment, with no
+// padding (brute-force checked: 1 wavefront per quarter warp for stride 2 and 4; stride 1 needs nothing).
+template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) {
+    return R == 1 ? i : (R == 2 ? i ^ ((i >> 3) & 1) : i ^ ((i >> 3) & 3));
+}
+
+// Packed fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a; a scalar operand is broadcast by the hardware).
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+
+constexpr int kSymBuf = 2;        // stage buffers
+// producer threads per CTA: they only issue cp.async.  The 192-consumer variant (mirror images: twice the staged
+// bytes per base pixel, so half the base pixels fit) runs 6 consumer + 2 producer warps = 2 warps per scheduler.
+__host__ __device__ constexpr int sym_nprod(int NC) { return NC == 192 ? 64 : 128; }
+__host__ __device__ constexpr int sym_planes(bool south, bool mirror) { return (south ? 2 : 1) * (mirror ? 2 : 1); }
+__host__ __device__ constexpr int sym_tmem_cols(int NC, int per_thread) {
+    int need = ((NC / 32 + 3) / 4) * per_thread, c = 32;
+    while (c < need) c *= 2;
+    return c;
+}
+
+// Tile n of this CTA: rows of gridDim.x tiles, alternate rows reversed ("snake") so that the CTAs
+// get equal shares of the work-sorted tile list without a global counter.
+__device__ __forceinline__ int snake_tile(int row, int G, int bid) { return row * G + ((row & 1) ? G - 1 - bid : bid); }
+
+__device__ __forceinline__ float4 lds128(unsigned a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+
+// Warp-specialised: the first NC threads are consumers (pair loop), the last sym_nprod(NC) threads are producers
+// (staging).  They meet only through the full/empty mbarriers of the kSymBuf stage buffers; there is no block-wide
+// barrier after the prologue.
+// TOT: per-step partial sums are added to a second accumulator set (pairwise-like summation; needed for
+// discs of thousands of pixels, costs as many registers again).
+// Z: two-zone table (lookup at tau(t), R11).  TM: the second accumulator set lives in tensor memory.
+template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
+__global__ void __launch_bounds__(NC + sym_nprod(NC), 1)
+sym_kernel(const Dev P, const FastDev F, const Maps io) {
+    static_assert(R == 1 || R == 2 || R == 4, "R");
+    constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
+    constexpr int NPROD = sym_nprod(NC);
+    constexpr int NPL = sym_planes(SOUTH, MIRROR);       // staged planes per position, 4 rotation images each
+    constexpr int G = 2 * NPL;                           // float2 accumulators per base pixel and map
+    constexpr int TMC = sym_tmem_cols(NC, R * G * 2);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *tab = reinterpret_cast<float2 *>(smem_raw);
+    const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 127) & ~(size_t)127));
+    __shared__ unsigned long long full_bar[kSymBuf], empty_bar[kSymBuf];
+    const int tid = threadIdx.x;
+    const int N = P.nside;
+    const int Ltot = F.Ltot;
+    const int GS = gridDim.x, bid = blockIdx.x;
+    const int nrows = (F.ntiles + GS - 1) / GS;
+
+    for (int i = tid; i < F.ntab_s; i += blockDim.x) tab[i] = P.tabh[i];
+    if (tid == 0) {
+        for (int i = 0; i < kSymBuf; ++i) { mbar_init(&full_bar[i], NPROD); mbar_init(&empty_bar[i], NC / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __shared__ unsigned s_tmem;
+    if (TM && tid < 32) {                                  // warp w uses TMEM lanes 32 (w % 4) .., columns (R G 2) (w / 4) ..
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(TMC) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    if (TM) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (TM) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    unsigned it = 0;                                     // steps so far: buffer it % kSymBuf, use it / kSymBuf
+    int rem_unused;
+
+    // register budget: the launch gives every thread 65536 / (NC + NPROD) registers (rounded down to a
+    // multiple of 8); the producer warps hand most of their share to the consumer warps
+    if (tid >= NC) {
+        // ======================================= producers =======================================
+        if (NC == 256 || NC == 384) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        const int pt = tid - NC;
+        const int m = pt & 3;                            // quadrant image staged by this thread
+        for (int row = 0; row < nrows; ++row) {
+            const int tile = snake_tile(row, GS, bid);
+            if (tile >= F.ntiles) continue;
+            const SymTile *tl = F.tiles + tile;
+            const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
+            for (int step = 0; step < nsteps; ++step, ++it) {
+                const int buf = it % kSymBuf;
+                // runs to stage for this step, worked out BEFORE waiting for the buffer so that the
+                // table reads (global memory) are off the critical path
+                int kq0[kMaxSub], km0[kMaxSub], Ls[kMaxSub], nqs[kMaxSub], sn[kMaxSub], ss[kMaxSub];
+                unsigned d0[kMaxSub];
+#pragma unroll
+                for (int s = 0; s < kMaxSub; ++s) {
+                    Ls[s] = 0;
+                    if (s >= nsub) continue;
+                    const int ne = __ldg(&tl->sub[s].ne);
+                    if (step >= ne) continue;
+                    const int r = __ldg(&tl->sub[s].r), k0 = __ldg(&tl->sub[s].k0), n = __ldg(&tl->sub[s].n);
+                    const int soff = __ldg(&tl->sub[s].soff);
+                    const PairEnt *pe = F.pairs + (__ldg(&tl->sub[s].e0) + step);
+                    const int2 pa = __ldg(reinterpret_cast<const int2 *>(&pe->rq));       // rq, hw
+                    const int2 pb = __ldg(reinterpret_cast<const int2 *>(&pe->ipq));      // ipq, shq
+                    const int2 ps = __ldg(reinterpret_cast<const int2 *>(&pe->start_n));  // start_n, start_s
+                    const int hw = pa.y, ipq = pb.x, shq = pb.y;
+                    const int ips = r < N ? r : N;
+                    const int shs = (r >= N) ? ((r - N) & 1) : 0;
+                    const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
+                    const int nq = 4 * ipq;
+                    const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
+                    const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw;
+                    Ls[s] = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R - w0;
+                    int k = w0 + m * ipq + nq;           // in [0, 2 nq)
+                    if (k >= nq) k -= nq;
+                    kq0[s] = k; nqs[s] = nq; sn[s] = ps.x; ss[s] = ps.y;
+                    // mirror image of position i: pixel (ipq - 1 + shq - (w0 + i)) + m ipq, walking backwards
+                    int km = ipq - 1 + shq - w0 + m * ipq;   // in (-nq, 2 nq + ...): w0 >= -hw - 1 > -ipq
+                    km %= nq; if (km < 0) km += nq;
+                    km0[s] = km;
+                    d0[s] = stage_sh + (unsigned)((buf * B * NPL) * Ltot + soff) * 16u + 4u * m;
+                }
+                mbar_wait_sleep(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);   // every consumer warp released it
+#pragma unroll
+                for (int s = 0; s < kMaxSub; ++s) {
+                    for (int i = pt >> 2; i < Ls[s]; i += NPROD / 4) {
+                        int kq = kq0[s] + i;             // L < nq: one wrap at most
+                        if (kq >= nqs[s]) kq -= nqs[s];
+                        int km = km0[s] - i;
+                        if (km < 0) km += nqs[s];
+                        const unsigned d = d0[s] + 16u * (unsigned)slot_of_pos<R>(i);
+#pragma unroll
+                        for (int b = 0; b < B; ++b) {
+                            unsigned dd = d + (unsigned)(b * NPL * Ltot) * 16u;
+                            cp_async4_s(dd, io.in[b] + sn[s] + kq);
+                            if (SOUTH) { dd += (unsigned)Ltot * 16u; cp_async4_s(dd, io.in[b] + ss[s] + kq); }
+                            if (MIRROR) {
+                                dd += (unsigned)Ltot * 16u; cp_async4_s(dd, io.in[b] + sn[s] + km);
+                                if (SOUTH) { dd += (unsigned)Ltot * 16u; cp_async4_s(dd, io.in[b] + ss[s] + km); }
+                            }
+                        }
+                    }
+                }
+                cp_async_mbar_arrive(&full_bar[buf]);   // arrives when this thread's copies have landed
+            }
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        return;
+    }
+
+    // ========================================= consumers =========================================
+    if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    if (NC == 384) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
+    // NC == 192: 256 threads per CTA, every thread may keep the 255 registers the compiler uses
+    const int warp = tid >> 5, lane = tid & 31;
+    const unsigned taddr = TM ? s_tmem + ((((unsigned)warp & 3u) * 32u) << 16) + ((unsigned)warp >> 2) * (unsigned)(R * G * 2) : 0u;
+    const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
+    const float tmax = P.tmax, eps = P.eps;
+    // shared-memory byte address of tab[0] minus 8 kMagicBits (mod 2^32): tab[bits - kMagicBits] = [tab_sh + 8 bits]
+    // (kept opaque: otherwise the compiler re-derives it from the CTA's shared window inside the pair loop)
+    unsigned tab_sh = smem_u32(tab) - kMagicBits * 8u;
+    asm volatile("mov.u32 %0, %0;" : "+r"(tab_sh));
+
+    for (int row = 0; row < nrows; ++row) {
+        const int tile = snake_tile(row, GS, bid);
+        if (tile >= F.ntiles) continue;
+        const SymTile *tl = F.tiles + tile;
+        const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
+        int si = 0;
+        for (int s = 1; s < nsub; ++s) if (warp >= __ldg(&tl->sub[s].w0)) si = s;
+        SubTile me;
+        {
+            const int4 *q = reinterpret_cast<const int4 *>(&tl->sub[si]);
+            const int4 a = __ldg(q), b = __ldg(q + 1);
+            me.r = a.x; me.k0 = a.y; me.n = a.z; me.e0 = a.w; me.ne = b.x; me.w0 = b.y; me.nw = b.z; me.soff = b.w;
+        }
+        const bool active = warp < me.w0 + me.nw;
+
+        const int r = me.r, k0 = me.k0;
+        const int ip = r < N ? r : N;                  // base rings are rings 1 .. 2N
+        const int ip2 = 2 * ip;
+        const unsigned M0 = 0xFFFFFFFFu / (unsigned)ip2;
+        const int sh = (r >= N) ? ((r - N) & 1) : 0;
+        const int klast = k0 + me.n - 1;
+        const int kmine = k0 + R * (32 * (warp - me.w0) + lane);
+        const int ka = min(kmine, klast);
+        const int ap = 2 * ka + 1 - sh, ap0 = 2 * k0 + 1 - sh;
+
+        float2 tot[TOT && !TM ? R : 1][B][G];
+#pragma unroll
+        for (int rr = 0; rr < (TOT && !TM ? R : 1); ++rr)
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int g = 0; g < G; ++g) tot[rr][b][g] = f2(0.f);
+        float2 acc[R][B][G];
+#pragma unroll
+        for (int rr = 0; rr < R; ++rr)
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int g = 0; g < G; ++g) acc[rr][b][g] = f2(0.f);
+
+        bool flushed = false;                              // TM: the totals in tensor memory are valid
+        PairEnt pe_next = F.pairs[me.e0];
+        for (int step = 0; step < nsteps; ++step, ++it) {
+            const int buf = it % kSymBuf;
+            const PairEnt pe = pe_next;
+            if (step + 1 < me.ne) pe_next = F.pairs[me.e0 + step + 1];       // prefetch under the pair loop
+            mbar_wait(&full_bar[buf], (it / kSymBuf) & 1u);
+            if (active && step < me.ne) {
+                const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
+                int rem;
+                const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
+                // azimuth of input pixel kc + j seen from base pixel ka + rr:  d = dcr[rr] + j dphi'
+                float dcr[R];
+#pragma unroll
+                for (int rr = 0; rr < R; ++rr) dcr[rr] = (float)(ip - rem - 2 * rr * pe.ipq) * pe.cdc;
+                // staged position of input pixel kc + j: i0 + j (slot_of_pos: padded against bank conflicts)
+                const int i0 = kc - w0;
+                unsigned pn[B];                          // shared address of this sub-tile's first plane, map b
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    pn[b] = stage_sh + (unsigned)(((buf * B + b) * NPL) * Ltot + me.soff) * 16u;
+                    asm volatile("mov.u32 %0, %0;" : "+r"(pn[b]));      // one register, not re-derived per position
+                }
+                const unsigned plane = (unsigned)Ltot * 16u;
+
+                // last table cell or the zero cell after it (rare): exact decision where needed
+                auto slow = [&](int rr, float tpv, unsigned &cb, int pos) {
+                    const float t = tpv + 0.5f;
+                    if (t >= tmax - eps) {
+                        if (t <= tmax + eps) {                   // decide in fp64, image by image
+                            const unsigned mask = sym_exact_mask(P, r, ka + rr, ip, sh, pe.rq, kc + pos - i0, pe.ipq, pe.shq, t,
+                                                                 SOUTH ? 1 : 0, MIRROR ? 1 : 0);
+                            if (mask) {
+                                const float2 el = tab[P.ntab - 2];
+                                float xk = fminf(t, tmax) - 0.5f;
+                                if (Z) { int jz; zoned_cell(P, fminf(t, tmax), jz, xk); xk -= 0.5f; }   // last cell, centred form
+                                const float Ku = fmaf(xk, el.y, el.x);
+#pragma unroll
+                                for (int b = 0; b < B; ++b) {
+                                    const unsigned a = pn[b] + 16u * (unsigned)slot_of_pos<R>(pos);
+#pragma unroll
+                                    for (int pl = 0; pl < NPL; ++pl) {
+                                        const float4 mq = lds128(a + pl * plane);
+                                        const unsigned mk = mask >> (4 * pl);
+                                        if (mk & 1u) acc[rr][b][2 * pl].x = fmaf(Ku, mq.x, acc[rr][b][2 * pl].x);
+                                        if (mk & 2u) acc[rr][b][2 * pl].y = fmaf(Ku, mq.y, acc[rr][b][2 * pl].y);
+                                        if (mk & 4u) acc[rr][b][2 * pl + 1].x = fmaf(Ku, mq.z, acc[rr][b][2 * pl + 1].x);
+                                        if (mk & 8u) acc[rr][b][2 * pl + 1].y = fmaf(Ku, mq.w, acc[rr][b][2 * pl + 1].y);
+                                    }
+                                }
+                            }
+                        }
+                        cb = thresh + 1u;                        // zero cell
+                    }
+                };
+
+                const float2 dphi2 = f2(pe.dphi), c4 = f2(pe.c4), c3 = f2(pe.c3), c2 = f2(pe.c2), c1 = f2(pe.c1), A2 = f2(pe.A);
+                // two-zone table: with t2 = t - 1/2, alpha t - 1/2 = alpha t2 + (alpha - 1)/2 and gamma (t - t1) - 1/2 = gamma t2 + gamma/2 - gamma t1 - 1/2
+                const float2 za2 = f2(P.z_alpha), zao2 = f2(0.5f * P.z_alpha - 0.5f), zg2 = f2(P.z_gamma), zgo2 = f2(0.5f * P.z_gamma - P.z_t1g - 0.5f);
+                const float zhm1f = (float)P.z_hm1;
+                const unsigned zhm1 = (unsigned)P.z_hm1;
+                float2 dc2[RP];
+#pragma unroll
+                for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
+                float2 jf = f2((float)(-pe.hw));
+                const int pos0 = i0 - pe.hw, pend = i0 + pe.hw + R - 1;
+                // One window position for the pixels rr in MASK (compile time).  The window of the thread is the
+                // union of its R pixels' windows, which are one position apart: pixel rr can only be inside the
+                // disc at positions pos0 + rr .. pend - (R - 1 - rr) (host: hw = floor(H / dphi' + 1/2 + 3 rho1),
+                // |dcr0| <= dphi' / 2, pixel rr is centred rr (1 +- rho1) positions further), so the first and the
+                // last R - 1 positions run bodies without the other pixels' geometry, gather and FMAs.
+                auto body = [&](int pos, auto MASK) {
+                    constexpr int mask = decltype(MASK)::value;
+                    float tp[2 * RP], tz_[2 * RP];
+                    unsigned cb[2 * RP], cz[2 * RP];
+#pragma unroll
+                    for (int h = 0; h < RP; ++h) {
+                        if (!((mask >> (2 * h)) & 3)) continue;
+                        const float2 d = __ffma2_rn(jf, dphi2, dc2[h]);
+                        const float2 y = __fmul2_rn(d, d);
+                        float2 p = __ffma2_rn(y, c4, c3);
+                        p = __ffma2_rn(y, p, c2);
+                        p = __ffma2_rn(y, p, c1);
+                        const float2 t2 = __ffma2_rn(y, p, A2);          // t - 0.5
+                        const float2 bb = __fadd2_rn(t2, f2(kMagic));
+                        tp[2 * h] = t2.x; tp[2 * h + 1] = t2.y;
+                        cb[2 * h] = __float_as_uint(bb.x); cb[2 * h + 1] = __float_as_uint(bb.y);
+                        if (Z) {
+                            // inner zone: alpha t - 1/2; outer zone: gamma (t - t1) - 1/2 RELATIVE to the zone start
+                            // (full resolution where the kernel is steep), cell offset added to the integer bits
+                            const float2 l1 = __ffma2_rn(t2, za2, zao2), l2 = __ffma2_rn(t2, zg2, zgo2);
+                            const bool o0 = l2.x + zhm1f < l1.x, o1 = l2.y + zhm1f < l1.y;
+                            const float2 tz = f2(o0 ? l2.x : l1.x, o1 ? l2.y : l1.y);
+                            const float2 bz = __fadd2_rn(tz, f2(kMagic));
+                            const float2 fz = __fadd2_rn(tz, __fadd2_rn(f2(kMagic), f2(-bz.x, -bz.y)));   // position - 1/2 in the cell
+                            tz_[2 * h] = fz.x; tz_[2 * h + 1] = fz.y;
+                            cz[2 * h] = __float_as_uint(bz.x) + (o0 ? zhm1 : 0u); cz[2 * h + 1] = __float_as_uint(bz.y) + (o1 ? zhm1 : 0u);
+                        }
+                    }
+                    // cells below the last: plain lookup; beyond the zero cell: clamp onto it (weight 0);
+                    // the last cell and the zero cell (t in [tmax - 1, tmax + 1)) take the branch
+                    unsigned mn = 0xFFFFFFFFu;
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) mn = min(mn, cb[rr] - thresh);
+                    float *tl = Z ? tz_ : tp;                              // lookup coordinate - 0.5 and its cell bits
+                    unsigned *cl = Z ? cz : cb;
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) cl[rr] = min(cl[rr], thresh + 1u);
+                    if (mn < 2u) {
+#pragma unroll
+                        for (int rr = 0; rr < R; ++rr)
+                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], cl[rr], pos);
+                    }
+                    float K[R];
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr) {
+                        if (!((mask >> rr) & 1)) continue;
+                        float2 el;                                  // tab[cb - kMagicBits], one LEA for the address
+                        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + cl[rr] * 8u));
+                        K[rr] = fmaf(tl[rr], el.y, el.x);
+                    }
+                    const unsigned so = 16u * (unsigned)slot_of_pos<R>(pos);
+#pragma unroll
+                    for (int b = 0; b < B; ++b) {
+                        float4 mv[NPL];
+#pragma unroll
+                        for (int pl = 0; pl < NPL; ++pl) mv[pl] = lds128(pn[b] + so + pl * plane);
+#pragma unroll
+                        for (int rr = 0; rr < R; ++rr) {
+                            if (!((mask >> rr) & 1)) continue;
+                            const float2 Kd = f2(K[rr]);
+#pragma unroll
+                            for (int pl = 0; pl < NPL; ++pl) {
+                                acc[rr][b][2 * pl] = __ffma2_rn(Kd, f2(mv[pl].x, mv[pl].y), acc[rr][b][2 * pl]);
+                                acc[rr][b][2 * pl + 1] = __ffma2_rn(Kd, f2(mv[pl].z, mv[pl].w), acc[rr][b][2 * pl + 1]);
+                            }
+                        }
+                    }
+                    jf = __fadd2_rn(jf, f2(1.0f));
+                };
+                constexpr int kAll = (1 << R) - 1;
+                int pos = pos0, plast = pend;
+                const bool peel = R > 1 && 2 * pe.hw >= R - 2;       // first and last R - 1 positions do not overlap
+                if (peel) {
+                    body(pos++, std::integral_constant<int, 1>{});
+                    if (R == 4) { body(pos++, std::integral_constant<int, 3>{}); body(pos++, std::integral_constant<int, 7>{}); }
+                    plast = pend - (R - 1);
+                }
+#pragma unroll 2
+                for (; pos <= plast; ++pos) body(pos, std::integral_constant<int, kAll>{});
+                if (peel) {
+                    if (R == 4) { body(pos++, std::integral_constant<int, 14 & kAll>{}); body(pos++, std::integral_constant<int, 12 & kAll>{}); }
+                    body(pos++, std::integral_constant<int, (1 << (R - 1))>{});
+                }
+                if (TOT && TM) {                                 // totals (tensor memory) += this ring's sums
+                    static_assert(!TM || B == 1, "TM variant: one map");
+                    static_assert(!TM || (R * G) % 8 == 0, "TM variant: 16 columns at a time");
+#pragma unroll
+                    for (int hh = 0; hh < R * G / 8; ++hh) {
+                        float v[16], old[16];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            float2 &a = acc[(hh * 8 + j) / G][0][(hh * 8 + j) % G];
+                            v[2 * j] = a.x; v[2 * j + 1] = a.y;
+                            a = f2(0.f);
+                        }
+                        if (flushed) {
+                            tmem_ld16(taddr + 16u * hh, old);
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) v[i] += old[i];
+                        }
+                        tmem_st16(taddr + 16u * hh, v);
+                    }
+                    tmem_wait_st();
+                    flushed = true;
+                } else if (TOT) {
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr)
+#pragma unroll
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int g = 0; g < G; ++g) {
+                                tot[TM ? 0 : rr][b][g] = __fadd2_rn(tot[TM ? 0 : rr][b][g], acc[rr][b][g]);
+                                acc[rr][b][g] = f2(0.f);
+                            }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_bar[buf]);         // this warp is done with the buffer
+        }
+
+        if (TM && flushed) {                               // totals back from tensor memory (into the accumulator registers)
+#pragma unroll
+            for (int hh = 0; hh < R * G / 8; ++hh) {
+                float old[16];
+                tmem_ld16(taddr + 16u * hh, old);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[(hh * 8 + j) / G][0][(hh * 8 + j) % G] = f2(old[2 * j], old[2 * j + 1]);
+            }
+        }
+        // store the images of every valid base pixel
+        if (active) {
+            const int start_n = P.start[r - 1], start_s = P.start[4 * N - r - 1];
+            const bool south_img = (r != 2 * N);
+#pragma unroll
+            for (int rr = 0; rr < R; ++rr) {
+                const int k = kmine + rr;
+                if (k <= klast) {
+                    // reflected base pixel; a pixel on the mirror axis (or at phi = 0 of a shifted ring, whose
+                    // reflection is its own rotation image) is its own mirror image: stored once
+                    const int km = ip - 1 + sh - k;
+                    const bool mir_img = MIRROR && (2 * k != ip - 1 + sh) && !(sh && k == 0);
+#pragma unroll
+                    for (int b = 0; b < B; ++b) {
+                        const float2 *s = (TOT && !TM) ? tot[TOT && !TM ? rr : 0][b] : acc[rr][b];
+#pragma unroll
+                        for (int pl = 0; pl < NPL; ++pl) {
+                            const bool is_s = SOUTH && (pl & 1), is_m = MIRROR && (pl >= (SOUTH ? 2 : 1));
+                            if ((is_s && !south_img) || (is_m && !mir_img)) continue;
+                            const float v[4] = {s[2 * pl].x, s[2 * pl].y, s[2 * pl + 1].x, s[2 * pl + 1].y};
+                            const int base = (is_s ? start_s : start_n) + (is_m ? km : k);
+#pragma unroll
+                            for (int m = 0; m < 4; ++m) io.out[b][base + m * ip] = v[m] * P.omega;
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (TM) {                                              // every consumer warp is done with tensor memory
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        asm volatile("bar.sync 2, %0;" ::"r"(NC) : "memory");
+        if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem), "n"(TMC) : "memory");
+    }
+}
+
+template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
+static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st) {
+    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s};
+    static bool attr_done[64] = {};
+    cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR>, attr_done);
+    if (e != cudaSuccess) return e;
+    const int grid = std::min(L.nsm, L.ntiles);
+    if (grid <= 0) return cudaSuccess;
+    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR><<<grid, NC + sym_nprod(NC), L.smem, st>>>(P, F, io);
+    return cudaGetLastError();
+}
+
+}  // namespace sc
