@@ -206,6 +206,24 @@ sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float 
                            float *const *out_maps, int B, void *cuda_stream);
 
 /*
+ * North polar cap only ("orienting the ... maps such that the survey area lies in the polar cap, reducing
+ * the number of rings"): a partial-sky map rotated so that the survey covers rings 1 .. ring_hi of the northern
+ * hemisphere.  sc_convolve_cap computes exactly those output rings; unlike a latitude band it evaluates NO southern
+ * mirror images (north-only kernel instance: 4 rotations x the reflection phi -> pi/2 - phi share a pair geometry) and
+ * reads nothing beyond the disc of ring ring_hi, so the map buffers need only hold the rows given by sc_cap_rows.
+ *
+ * sc_cap_rows -- HOST outputs (may be NULL): out_rows[2] = pixel range [0, o1) written (rings 1 .. ring_hi),
+ *   in_rows[2] = pixel range [0, i1) read (rings up to ring_hi + theta_max overlap).  1 <= ring_hi <= 2 nside.
+ * sc_convolve_cap -- in_maps / out_maps: HOST arrays of B DEVICE pointers to at least in_rows[1] / out_rows[1] fp32
+ *   values (RING order from the north pole), 16-byte aligned, not overlapping.  Pixels >= out_rows[1] are not touched.
+ *   Maps are processed one per launch.  RING plans only (SC_ERR_UNSUPPORTED for NESTED).  The first call for a new
+ *   ring_hi builds its tile list (synchronous); later calls are asynchronous on the stream.
+ */
+sc_status sc_cap_rows(const sc_plan *plan, int ring_hi, int64_t *out_rows, int64_t *in_rows);
+sc_status sc_convolve_cap(sc_plan *plan, int ring_hi, const float *const *in_maps, float *const *out_maps, int B,
+                          void *cuda_stream);
+
+/*
  * sc_debug_fma_peak -- measurement only: the sustained FP32 FMA rate of the current device, measured with a
  * register-only loop of independent FMA chains (packed = 0: scalar FFMA; packed = 1: FFMA2, the packed form the
  * convolution kernels accumulate with) on 2 x 1024 threads per SM, best of 3 launches of a few ms.  bench.py uses

@@ -14,7 +14,7 @@ SC_K_POLAR, SC_K_SYM, SC_K_BELT, SC_K_COUNT = 0, 1, 2, 3
 KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
 
 EXPORTS = ("sc_plan_create", "sc_plan_create_zoned", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
-           "sc_band_partition", "sc_convolve_band",
+           "sc_band_partition", "sc_convolve_band", "sc_cap_rows", "sc_convolve_cap",
            "sc_plan_destroy", "sc_plan_set_path",
            "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_debug_fma_peak", "sc_last_launch_count",
            "sc_status_string", "sc_last_cuda_error", "sc_version")
@@ -48,6 +48,8 @@ def lib():
         l.sc_plan_partition.argtypes = [vp, vp, vp]
         l.sc_band_partition.argtypes = [vp, i32, i32, vp, vp, vp, vp]
         l.sc_convolve_band.argtypes = [vp, i32, i32, vp, vp, i32, vp]
+        l.sc_cap_rows.argtypes = [vp, i32, vp, vp]
+        l.sc_convolve_cap.argtypes = [vp, i32, vp, vp, i32, vp]
         l.sc_plan_destroy.argtypes = [vp]
         l.sc_plan_set_path.argtypes = [vp, i32]
         l.sc_plan_info.argtypes = [vp, vp, vp, vp, vp]
@@ -140,6 +142,21 @@ def sc_convolve_band(plan, ring_lo, ring_hi, in_ptrs, out_ptrs, stream=0):
         raise ValueError("in/out batch mismatch")
     _chk(lib().sc_convolve_band(plan, int(ring_lo), int(ring_hi), _ptr_array(in_ptrs), _ptr_array(out_ptrs),
                                 len(in_ptrs), C.c_void_p(int(stream) or None)), "sc_convolve_band")
+
+
+def sc_cap_rows(plan, ring_hi):
+    """-> dict(out_rows=(0, o1), in_rows=(0, i1)): pixel ranges written / read by sc_convolve_cap(ring_hi)."""
+    orow, irow = (C.c_int64 * 2)(), (C.c_int64 * 2)()
+    _chk(lib().sc_cap_rows(plan, int(ring_hi), orow, irow), "sc_cap_rows")
+    return dict(out_rows=tuple(orow), in_rows=tuple(irow))
+
+
+def sc_convolve_cap(plan, ring_hi, in_ptrs, out_ptrs, stream=0):
+    """North polar cap only: output rings 1 .. ring_hi, no southern mirror images (include/sc.h)."""
+    if len(in_ptrs) != len(out_ptrs):
+        raise ValueError("in/out batch mismatch")
+    _chk(lib().sc_convolve_cap(plan, int(ring_hi), _ptr_array(in_ptrs), _ptr_array(out_ptrs), len(in_ptrs),
+                               C.c_void_p(int(stream) or None)), "sc_convolve_cap")
 
 
 def sc_plan_destroy(plan):
@@ -242,6 +259,16 @@ class Plan:
         import torch
         sc_convolve_band(self.handle, ring_lo, ring_hi, [m.data_ptr() for m in maps], [o.data_ptr() for o in out],
                          torch.cuda.current_stream().cuda_stream)
+        return out
+
+    def cap_rows(self, ring_hi):
+        return sc_cap_rows(self.handle, ring_hi)
+
+    def convolve_cap(self, ring_hi, maps, out):
+        """North polar cap only: maps / out are CUDA fp32 tensors holding at least the rows of cap_rows(ring_hi)."""
+        import torch
+        sc_convolve_cap(self.handle, ring_hi, [m.data_ptr() for m in maps], [o.data_ptr() for o in out],
+                        torch.cuda.current_stream().cuda_stream)
         return out
 
     def convolve_host(self, maps, out=None):

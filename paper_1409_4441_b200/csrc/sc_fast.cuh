@@ -40,6 +40,7 @@ struct FastDev {
     int ntiles;
     int Ltot;               // staged positions per plane
     int ntab_s;             // entries of the shared-memory table
+    int dbg;                // measurement only (SC_DBG): 1 = consumers skip the pair loop, 2 = producers skip the copies
 };
 
 // What a launch of the sym kernel needs from the plan (host); the instantiations live in sc_sym_b1.cu (one map per

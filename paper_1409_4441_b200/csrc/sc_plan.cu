@@ -29,6 +29,7 @@ cudaError_t reorder_i32(int nside, int dir, const int *src, int *dst, cudaStream
 cudaError_t reorder_u64(int nside, int dir, const unsigned long long *src, unsigned long long *dst, cudaStream_t st);
 cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, int lo, int hi, cudaStream_t st, int *launches);
 void fast_chunk_rings(const FastPlan *fp, int B, int kind, int i, int *lo, int *hi);
+cudaError_t fast_launch_cap(FastPlan *fp, const Dev &P, const Maps &io, int ring_hi, cudaStream_t st, int *launches);
 bool fast_available(const FastPlan *fp, int B);
 }  // namespace sc
 
@@ -682,6 +683,61 @@ sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float 
         }
         int nl = 0;
         SC_CUDA(sc::fast_launch_band(plan->fast, D, io, nb, ring_lo, ring_hi, st, &nl));
+        launches += nl;
+    }
+    plan->last_launches = launches;
+    return SC_OK;
+}
+
+sc_status sc_cap_rows(const sc_plan *plan, int ring_hi, int64_t *out_rows, int64_t *in_rows) {
+    if (!plan) return SC_ERR_INVALID_ARG;
+    const int N = plan->dev.nside, N4 = 4 * N;
+    if (ring_hi < 1 || ring_hi > 2 * N) return SC_ERR_INVALID_ARG;
+    auto row = [&](int ring) -> int64_t { return ring <= N4 - 1 ? (int64_t)plan->rings[ring - 1].start : (int64_t)plan->dev.npix; };
+    if (out_rows) { out_rows[0] = 0; out_rows[1] = row(ring_hi + 1); }
+    if (in_rows) { in_rows[0] = 0; in_rows[1] = row(std::min(N4 - 1, plan->rhi_h[ring_hi - 1] + 1) + 1); }
+    return SC_OK;
+}
+
+sc_status sc_convolve_cap(sc_plan *plan, int ring_hi, const float *const *in_maps, float *const *out_maps, int B,
+                          void *cuda_stream) {
+    if (!plan || !in_maps || !out_maps || B < 1) return SC_ERR_INVALID_ARG;
+    const sc::Dev &D = plan->dev;
+    const int N = D.nside;
+    if (ring_hi < 1 || ring_hi > 2 * N) return SC_ERR_INVALID_ARG;
+    if (plan->nested) return SC_ERR_UNSUPPORTED;                       // a cap is a contiguous block of rows in RING order only
+    int64_t orow[2], irow[2];
+    sc_cap_rows(plan, ring_hi, orow, irow);
+    // the maps need only exist up to the last row read / written: overlap is checked on those extents
+    for (int b = 0; b < B; ++b) {
+        if (!in_maps[b] || !out_maps[b]) return SC_ERR_INVALID_ARG;
+        if (((uintptr_t)in_maps[b] | (uintptr_t)out_maps[b]) & 15u) return SC_ERR_INVALID_ARG;
+    }
+    for (int b = 0; b < B; ++b)
+        for (int a = 0; a < B; ++a) {
+            const uintptr_t o0 = (uintptr_t)out_maps[b], o1 = o0 + (uintptr_t)orow[1] * 4;
+            const uintptr_t i0 = (uintptr_t)in_maps[a], i1 = i0 + (uintptr_t)irow[1] * 4;
+            if (o0 < i1 && i0 < o1) return SC_ERR_INVALID_ARG;
+            const uintptr_t p0 = (uintptr_t)out_maps[a], p1 = p0 + (uintptr_t)orow[1] * 4;
+            if (a != b && o0 < p1 && p0 < o1) return SC_ERR_INVALID_ARG;
+        }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int launches = 0;
+    for (int b = 0; b < B; ++b) {                                      // one map per launch (north-only kernel instance)
+        sc::Maps io{};
+        io.in[0] = in_maps[b]; io.out[0] = out_maps[b];
+        if (plan->path == SC_PATH_GENERIC || !plan->fast) {
+            SC_CUDA(sc::launch_generic_conv(D, io, 1, 0, (int)orow[1], 0, 0, st));
+            ++launches;
+            continue;
+        }
+        const int pr = std::min(plan->polar_rings, ring_hi);
+        if (pr > 0) {                                                  // rings next to the pole
+            SC_CUDA(sc::launch_generic_conv_warp(D, io, 1, 0, 2 * pr * (pr + 1), 0, 0, st));
+            ++launches;
+        }
+        int nl = 0;
+        SC_CUDA(sc::fast_launch_cap(plan->fast, D, io, ring_hi, st, &nl));
         launches += nl;
     }
     plan->last_launches = launches;

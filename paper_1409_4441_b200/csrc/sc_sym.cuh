@@ -30,6 +30,7 @@
 #include "sc_fast.cuh"
 
 #include <algorithm>
+#include <cstdlib>
 #include <type_traits>
 
 namespace sc {
@@ -83,16 +84,36 @@ template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) {
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
 
+// &base[idx] with one IMAD.WIDE.U32
+__device__ __forceinline__ const float *elem_ptr(const float *base, unsigned idx) {
+    unsigned long long a;
+    asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(a) : "r"(idx), "l"(base));
+    return reinterpret_cast<const float *>(a);
+}
+
 constexpr int kSymBuf = 2;        // stage buffers
-// producer threads per CTA: they only issue cp.async.  The 192-consumer variant (mirror images: twice the staged
-// bytes per base pixel, so half the base pixels fit) runs 6 consumer + 2 producer warps = 2 warps per scheduler.
-__host__ __device__ constexpr int sym_nprod(int NC) { return NC == 192 ? 64 : 128; }
+// Producer threads per CTA: they only issue cp.async.  One warpgroup, except in the 192-consumer variant (mirror
+// images: twice the staged bytes per base pixel, so half the base pixels fit): 6 consumer + 2 producer warps, i.e. two
+// warps on every scheduler, 256 threads that keep the compiler's register count (no setmaxnreg).
+#ifndef SC_L192
+#define SC_L192 1
+#endif
+__host__ __device__ constexpr int sym_nprod(int NC) { return (NC == 192 && SC_L192 == 1) ? 64 : 128; }
+// SC_L192 == 0 (A/B layout): warps 0-5 = consumers, 6-7 = idle (they exit after the register hand-over of their
+// warpgroup: setmaxnreg works on whole warpgroups), 8-11 = producers.
+__host__ __device__ constexpr int sym_prod0(int NC) { return (NC == 192 && SC_L192 == 0) ? 256 : NC; }     // first producer thread
+__host__ __device__ constexpr int sym_threads(int NC) { return sym_prod0(NC) + sym_nprod(NC); }
 __host__ __device__ constexpr int sym_planes(bool south, bool mirror) { return (south ? 2 : 1) * (mirror ? 2 : 1); }
 __host__ __device__ constexpr int sym_tmem_cols(int NC, int per_thread) {
     int need = ((NC / 32 + 3) / 4) * per_thread, c = 32;
     while (c < need) c *= 2;
     return c;
 }
+
+// Per-position state of the pair loop: lookup coordinate - 1/2 and table cell bits of the R pixels (geometry stage),
+// table cells and map values (load stage)
+template <int R> struct SymGeo { float t[R < 2 ? 2 : R]; unsigned c[R < 2 ? 2 : R]; };
+template <int R, int B, int NPL> struct SymLd { float2 el[R]; float4 mv[B][NPL]; };
 
 // Tile n of this CTA: rows of gridDim.x tiles, alternate rows reversed ("snake") so that the CTAs
 // get equal shares of the work-sorted tile list without a global counter.
@@ -111,11 +132,11 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 // discs of thousands of pixels, costs as many registers again).
 // Z: two-zone table (lookup at tau(t), R11).  TM: the second accumulator set lives in tensor memory.
 template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
-__global__ void __launch_bounds__(NC + sym_nprod(NC), 1)
+__global__ void __launch_bounds__(sym_threads(NC), 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(R == 1 || R == 2 || R == 4, "R");
     constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
-    constexpr int NPROD = sym_nprod(NC);
+    constexpr int NPROD = sym_nprod(NC), PROD0 = sym_prod0(NC);
     constexpr int NPL = sym_planes(SOUTH, MIRROR);       // staged planes per position, 4 rotation images each
     constexpr int G = 2 * NPL;                           // float2 accumulators per base pixel and map
     constexpr int TMC = sym_tmem_cols(NC, R * G * 2);
@@ -145,12 +166,12 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     unsigned it = 0;                                     // steps so far: buffer it % kSymBuf, use it / kSymBuf
     int rem_unused;
 
-    // register budget: the launch gives every thread 65536 / (NC + NPROD) registers (rounded down to a
-    // multiple of 8); the producer warps hand most of their share to the consumer warps
-    if (tid >= NC) {
+    // register budget: the launch gives every thread 65536 / blockDim.x registers (rounded down to a
+    // multiple of 8); the producer warpgroup hands most of its share to the consumer warpgroups
+    if (tid >= PROD0) {
         // ======================================= producers =======================================
-        if (NC == 256 || NC == 384) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
-        const int pt = tid - NC;
+        if (NC == 256 || NC == 384 || (NC == 192 && SC_L192 == 0)) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+        const int pt = tid - PROD0;
         const int m = pt & 3;                            // quadrant image staged by this thread
         for (int row = 0; row < nrows; ++row) {
             const int tile = snake_tile(row, GS, bid);
@@ -195,21 +216,45 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 mbar_wait_sleep(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);   // every consumer warp released it
 #pragma unroll
                 for (int s = 0; s < kMaxSub; ++s) {
-                    for (int i = pt >> 2; i < Ls[s]; i += NPROD / 4) {
-                        int kq = kq0[s] + i;             // L < nq: one wrap at most
-                        if (kq >= nqs[s]) kq -= nqs[s];
-                        int km = km0[s] - i;
-                        if (km < 0) km += nqs[s];
-                        const unsigned d = d0[s] + 16u * (unsigned)slot_of_pos<R>(i);
+                    if (F.dbg & 2) break;
+                    // this thread's positions i = pt / 4 + j NPROD / 4: input pixel kq walks forwards, its mirror
+                    // image km backwards, both with at most one wrap (L < nq); unsigned 32-bit indices added to
+                    // the ring's base pointer keep the address arithmetic to one instruction per copy
+                    const unsigned nq = (unsigned)nqs[s];
+                    int i = pt >> 2;
+                    unsigned kq = (unsigned)(kq0[s] + i); if (kq >= nq) kq -= nq;
+                    int km = km0[s] - i; if (km < 0) km += (int)nq;
+                    const unsigned plane = (unsigned)Ltot * 16u;
+                    const float *gn[B], *gs[B];              // first pixel of the input ring and of its southern mirror
 #pragma unroll
-                        for (int b = 0; b < B; ++b) {
-                            unsigned dd = d + (unsigned)(b * NPL * Ltot) * 16u;
-                            cp_async4_s(dd, io.in[b] + sn[s] + kq);
-                            if (SOUTH) { dd += (unsigned)Ltot * 16u; cp_async4_s(dd, io.in[b] + ss[s] + kq); }
-                            if (MIRROR) {
-                                dd += (unsigned)Ltot * 16u; cp_async4_s(dd, io.in[b] + sn[s] + km);
-                                if (SOUTH) { dd += (unsigned)Ltot * 16u; cp_async4_s(dd, io.in[b] + ss[s] + km); }
+                    for (int b = 0; b < B; ++b) {
+                        gn[b] = io.in[b] + sn[s]; gs[b] = io.in[b] + ss[s];
+                        asm volatile("" : "+l"(gn[b]), "+l"(gs[b]));     // kept as 64-bit registers
+                    }
+                    // positions 32 apart share the swizzle term of slot_of_pos: the destinations advance by 512 bytes per
+                    // iteration; a thread takes PPI positions (NPROD / 4 apart) per iteration
+                    constexpr int PPI = 32 / (NPROD / 4);
+                    static_assert(PPI == 1 || PPI == 2, "positions per producer iteration");
+                    unsigned d = d0[s] + 16u * (unsigned)slot_of_pos<R>(i);
+                    const unsigned d2off = 16u * (unsigned)slot_of_pos<R>(i + NPROD / 4) - 16u * (unsigned)slot_of_pos<R>(i);
+                    const int L = Ls[s];
+#pragma unroll 2
+                    for (; i < L; i += 32, d += 512u) {
+#pragma unroll
+                        for (int u = 0; u < PPI; ++u) {
+                            if (u == 1 && i + NPROD / 4 >= L) break;
+#pragma unroll
+                            for (int b = 0; b < B; ++b) {
+                                unsigned dd = d + (u ? d2off : 0u) + (unsigned)(b * NPL) * plane;
+                                cp_async4_s(dd, elem_ptr(gn[b], kq));
+                                if (SOUTH) { dd += plane; cp_async4_s(dd, elem_ptr(gs[b], kq)); }
+                                if (MIRROR) {
+                                    dd += plane; cp_async4_s(dd, elem_ptr(gn[b], (unsigned)km));
+                                    if (SOUTH) { dd += plane; cp_async4_s(dd, elem_ptr(gs[b], (unsigned)km)); }
+                                }
                             }
+                            kq += NPROD / 4; if (kq >= nq) kq -= nq;
+                            km -= NPROD / 4; if (km < 0) km += (int)nq;
                         }
                     }
                 }
@@ -223,7 +268,10 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     // ========================================= consumers =========================================
     if (NC == 256) asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
     if (NC == 384) asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
-    // NC == 192: 256 threads per CTA, every thread may keep the 255 registers the compiler uses
+    if (NC == 192 && SC_L192 == 0) {                       // 384 threads x 168 registers = 256 x 224 + 128 x 56
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+        if (tid >= NC) return;                             // warps 6-7 only complete the warpgroup
+    }
     const int warp = tid >> 5, lane = tid & 31;
     const unsigned taddr = TM ? s_tmem + ((((unsigned)warp & 3u) * 32u) << 16) + ((unsigned)warp >> 2) * (unsigned)(R * G * 2) : 0u;
     const unsigned thresh = kMagicBits + (unsigned)(P.ntab - 2);   // bits of the last table cell
@@ -280,7 +328,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             const PairEnt pe = pe_next;
             if (step + 1 < me.ne) pe_next = F.pairs[me.e0 + step + 1];       // prefetch under the pair loop
             mbar_wait(&full_bar[buf], (it / kSymBuf) & 1u);
-            if (active && step < me.ne) {
+            if (active && step < me.ne && !(F.dbg & 1)) {
                 const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
                 int rem;
                 const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
@@ -344,10 +392,18 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 // disc at positions pos0 + rr .. pend - (R - 1 - rr) (host: hw = floor(H / dphi' + 1/2 + 3 rho1),
                 // |dcr0| <= dphi' / 2, pixel rr is centred rr (1 +- rho1) positions further), so the first and the
                 // last R - 1 positions run bodies without the other pixels' geometry, gather and FMAs.
-                auto body = [&](int pos, auto MASK) {
+                // The work of one position in three stages, so that the main loop can be software-pipelined (with only
+                // 6-12 consumer warps per SM the shared-memory latency must be covered inside the warp):
+                //   geom: pair geometry -> lookup coordinate - 1/2 (gt) and table cell bits (gc) of the R pixels,
+                //         exact fp64 decisions for the rare cells next to theta_max (slow);
+                //   load: the table cells (one LDS.64 gather per pixel) and the map values of this position;
+                //   fma:  K = a + t b and the accumulation into the images.
+                auto geom = [&](int pos, auto MASK, SymGeo<R> &ge) {
+                    float *gt = ge.t;
+                    unsigned *gc = ge.c;
                     constexpr int mask = decltype(MASK)::value;
-                    float tp[2 * RP], tz_[2 * RP];
-                    unsigned cb[2 * RP], cz[2 * RP];
+                    float tp[2 * RP];
+                    unsigned cb[2 * RP];
 #pragma unroll
                     for (int h = 0; h < RP; ++h) {
                         if (!((mask >> (2 * h)) & 3)) continue;
@@ -360,6 +416,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         const float2 bb = __fadd2_rn(t2, f2(kMagic));
                         tp[2 * h] = t2.x; tp[2 * h + 1] = t2.y;
                         cb[2 * h] = __float_as_uint(bb.x); cb[2 * h + 1] = __float_as_uint(bb.y);
+                        gt[2 * h] = t2.x; gt[2 * h + 1] = t2.y;
+                        gc[2 * h] = cb[2 * h]; gc[2 * h + 1] = cb[2 * h + 1];
                         if (Z) {
                             // inner zone: alpha t - 1/2; outer zone: gamma (t - t1) - 1/2 RELATIVE to the zone start
                             // (full resolution where the kernel is steep), cell offset added to the integer bits
@@ -368,8 +426,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                             const float2 tz = f2(o0 ? l2.x : l1.x, o1 ? l2.y : l1.y);
                             const float2 bz = __fadd2_rn(tz, f2(kMagic));
                             const float2 fz = __fadd2_rn(tz, __fadd2_rn(f2(kMagic), f2(-bz.x, -bz.y)));   // position - 1/2 in the cell
-                            tz_[2 * h] = fz.x; tz_[2 * h + 1] = fz.y;
-                            cz[2 * h] = __float_as_uint(bz.x) + (o0 ? zhm1 : 0u); cz[2 * h + 1] = __float_as_uint(bz.y) + (o1 ? zhm1 : 0u);
+                            gt[2 * h] = fz.x; gt[2 * h + 1] = fz.y;
+                            gc[2 * h] = __float_as_uint(bz.x) + (o0 ? zhm1 : 0u); gc[2 * h + 1] = __float_as_uint(bz.y) + (o1 ? zhm1 : 0u);
                         }
                     }
                     // cells below the last: plain lookup; beyond the zero cell: clamp onto it (weight 0);
@@ -377,43 +435,58 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     unsigned mn = 0xFFFFFFFFu;
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) mn = min(mn, cb[rr] - thresh);
-                    float *tl = Z ? tz_ : tp;                              // lookup coordinate - 0.5 and its cell bits
-                    unsigned *cl = Z ? cz : cb;
 #pragma unroll
-                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) cl[rr] = min(cl[rr], thresh + 1u);
+                    for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) gc[rr] = min(gc[rr], thresh + 1u);
                     if (mn < 2u) {
 #pragma unroll
                         for (int rr = 0; rr < R; ++rr)
-                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], cl[rr], pos);
-                    }
-                    float K[R];
-#pragma unroll
-                    for (int rr = 0; rr < R; ++rr) {
-                        if (!((mask >> rr) & 1)) continue;
-                        float2 el;                                  // tab[cb - kMagicBits], one LEA for the address
-                        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el.x), "=f"(el.y) : "r"(tab_sh + cl[rr] * 8u));
-                        K[rr] = fmaf(tl[rr], el.y, el.x);
-                    }
-                    const unsigned so = 16u * (unsigned)slot_of_pos<R>(pos);
-#pragma unroll
-                    for (int b = 0; b < B; ++b) {
-                        float4 mv[NPL];
-#pragma unroll
-                        for (int pl = 0; pl < NPL; ++pl) mv[pl] = lds128(pn[b] + so + pl * plane);
-#pragma unroll
-                        for (int rr = 0; rr < R; ++rr) {
-                            if (!((mask >> rr) & 1)) continue;
-                            const float2 Kd = f2(K[rr]);
-#pragma unroll
-                            for (int pl = 0; pl < NPL; ++pl) {
-                                acc[rr][b][2 * pl] = __ffma2_rn(Kd, f2(mv[pl].x, mv[pl].y), acc[rr][b][2 * pl]);
-                                acc[rr][b][2 * pl + 1] = __ffma2_rn(Kd, f2(mv[pl].z, mv[pl].w), acc[rr][b][2 * pl + 1]);
-                            }
-                        }
+                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], gc[rr], pos);
                     }
                     jf = __fadd2_rn(jf, f2(1.0f));
                 };
+                auto load = [&](int pos, auto MASK, const SymGeo<R> &ge, SymLd<R, B, NPL> &ld) {
+                    const unsigned *gc = ge.c;
+                    float2 *el = ld.el;
+                    float4 (*mv)[NPL] = ld.mv;
+                    constexpr int mask = decltype(MASK)::value;
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr) {
+                        if (!((mask >> rr) & 1)) continue;          // tab[gc - kMagicBits], one LEA for the address
+                        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el[rr].x), "=f"(el[rr].y) : "r"(tab_sh + gc[rr] * 8u));
+                    }
+                    const unsigned so = 16u * (unsigned)slot_of_pos<R>(pos);
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int pl = 0; pl < NPL; ++pl) mv[b][pl] = lds128(pn[b] + so + pl * plane);
+                };
+                auto fma = [&](auto MASK, const SymGeo<R> &ge, const SymLd<R, B, NPL> &ld) {
+                    const float *gt = ge.t;
+                    const float2 *el = ld.el;
+                    const float4 (*mv)[NPL] = ld.mv;
+                    constexpr int mask = decltype(MASK)::value;
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr) {
+                        if (!((mask >> rr) & 1)) continue;
+                        const float2 Kd = f2(fmaf(gt[rr], el[rr].y, el[rr].x));
+#pragma unroll
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int pl = 0; pl < NPL; ++pl) {
+                                acc[rr][b][2 * pl] = __ffma2_rn(Kd, f2(mv[b][pl].x, mv[b][pl].y), acc[rr][b][2 * pl]);
+                                acc[rr][b][2 * pl + 1] = __ffma2_rn(Kd, f2(mv[b][pl].z, mv[b][pl].w), acc[rr][b][2 * pl + 1]);
+                            }
+                    }
+                };
+                SymGeo<R> geA, geB;
+                SymLd<R, B, NPL> ldA, ldB;
+                auto body = [&](int pos, auto MASK) {             // one position, not pipelined (window edges)
+                    geom(pos, MASK, geA);
+                    load(pos, MASK, geA, ldA);
+                    fma(MASK, geA, ldA);
+                };
                 constexpr int kAll = (1 << R) - 1;
+                const auto ALL = std::integral_constant<int, kAll>{};
                 int pos = pos0, plast = pend;
                 const bool peel = R > 1 && 2 * pe.hw >= R - 2;       // first and last R - 1 positions do not overlap
                 if (peel) {
@@ -421,8 +494,31 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     if (R == 4) { body(pos++, std::integral_constant<int, 3>{}); body(pos++, std::integral_constant<int, 7>{}); }
                     plast = pend - (R - 1);
                 }
+                // Main positions (all R pixels), software-pipelined over two register sets: the loads of position
+                // i + 1 are issued before the FMAs of position i, the geometry of position i + 2 after them.  The
+                // number of positions is the same for all lanes (2 hw + R - 2 (R - 1) or 2 hw + R).
+                int left = plast - pos + 1;
+                constexpr bool PIPE = NC != 384;                     // 384 consumers: 152 registers per thread, no room
+                if (!PIPE) {
 #pragma unroll 2
-                for (; pos <= plast; ++pos) body(pos, std::integral_constant<int, kAll>{});
+                    for (; pos <= plast; ++pos) body(pos, ALL);
+                } else if (left > 0) {
+                    geom(pos, ALL, geA);
+                    load(pos, ALL, geA, ldA);
+                    if (left > 1) geom(pos + 1, ALL, geB);
+                    while (true) {
+                        if (left > 1) load(pos + 1, ALL, geB, ldB);
+                        fma(ALL, geA, ldA);
+                        if (left > 2) geom(pos + 2, ALL, geA);
+                        ++pos;
+                        if (--left == 0) break;
+                        if (left > 1) load(pos + 1, ALL, geA, ldA);
+                        fma(ALL, geB, ldB);
+                        if (left > 2) geom(pos + 2, ALL, geB);
+                        ++pos;
+                        if (--left == 0) break;
+                    }
+                }
                 if (peel) {
                     if (R == 4) { body(pos++, std::integral_constant<int, 14 & kAll>{}); body(pos++, std::integral_constant<int, 12 & kAll>{}); }
                     body(pos++, std::integral_constant<int, (1 << (R - 1))>{});
@@ -511,13 +607,14 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 
 template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
 static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st) {
-    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s};
+    const char *dbg = std::getenv("SC_DBG");
+    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0};
     static bool attr_done[64] = {};
     cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = std::min(L.nsm, L.ntiles);
     if (grid <= 0) return cudaSuccess;
-    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR><<<grid, NC + sym_nprod(NC), L.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 

@@ -11,7 +11,8 @@ cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cu
 #define SC_GO(R, NC, TOT, TM, SOUTH, MIRROR) \
     return z ? launch_sym<1, R, NC, TOT, true, TM, SOUTH, MIRROR>(L, P, io, st) : launch_sym<1, R, NC, TOT, false, TM, SOUTH, MIRROR>(L, P, io, st)
     if (L.south && L.mirror) {                          // 16 images
-        if (L.threads == 192 && L.R == 4 && !L.tmem) { if (L.tot) { SC_GO(4, 192, true, false, true, true); } else { SC_GO(4, 192, false, false, true, true); } }
+        if (L.threads == 192 && L.R == 4 && L.tot && L.tmem) { SC_GO(4, 192, true, true, true, true); }
+        if (L.threads == 192 && L.R == 4 && !L.tot && !L.tmem) { SC_GO(4, 192, false, false, true, true); }
         return cudaErrorInvalidValue;
     }
     if (!L.south && L.mirror) {                         // north only, 8 images

@@ -470,6 +470,61 @@ def test_bands_with_simulated_halo_exchange(sc, ci, world, B):
             assert torch.equal(o, f)
 
 
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("ci,frac,B", [(1, 0.3, 1), (1, 1.0, 2), (2, 0.5, 1), (3, 0.45, 1), (3, 0.97, 2), (4, 0.3, 1)])
+def test_north_cap_only(sc, path, ci, frac, B):
+    """sc_convolve_cap (the survey area rotated into the polar cap): output rings 1 .. ring_hi only, from
+    TRUNCATED buffers that hold just the rows sc_cap_rows names (NaN guard words after the input, a sentinel after the
+    output): nothing beyond is read or written, no southern mirror is computed, values and -- with K == 1 and integer
+    maps -- the neighbour sets equal the oracle's."""
+    import torch
+    cfg = gen.config(ci)
+    N = cfg.nside
+    if path == "generic" and N > 1024:
+        pytest.skip("generic path at Nside 2048: minutes")
+    ring_hi = max(1, min(2 * N, int(round(frac * 2 * N))))
+    T = gen.table_for(cfg)
+    maps = [gen.noise_map(cfg.npix, 1200 + 10 * ci + b) for b in range(B)]
+    imaps = [np.random.default_rng(77 + b).integers(-8, 9, size=cfg.npix).astype(np.float32) for b in range(B)]
+    tb = O.ring_table(N)
+    for table, inputs, exact in ((T, maps, False), (np.ones(cfg.n_table), imaps, True)):
+        with sc.Plan(N, table, cfg.theta_max, B) as plan:
+            _set_path(sc, plan, path)
+            rows = plan.cap_rows(ring_hi)
+            o1, i1 = rows["out_rows"][1], rows["in_rows"][1]
+            assert rows["out_rows"][0] == 0 and rows["in_rows"][0] == 0 and o1 <= i1 <= cfg.npix
+            assert o1 == int(tb["start"][ring_hi - 1] + tb["npr"][ring_hi - 1])
+            bin_, bout = [], []
+            for m in inputs:
+                t = torch.full((i1 + 64,), float("nan"), dtype=torch.float32, device="cuda")
+                t[:i1] = torch.from_numpy(m[:i1]).cuda()
+                bin_.append(t)
+                bout.append(torch.full((o1 + 64,), -777.0, dtype=torch.float32, device="cuda"))
+            plan.convolve_cap(ring_hi, bin_, bout)
+            plan.convolve_cap(ring_hi, bin_, bout)                    # cached tile list, same result
+            torch.cuda.synchronize()
+            part = plan.partition()
+        rings = sorted({1, 2, max(1, min(part["polar_rings"], ring_hi)), min(part["polar_rings"] + 1, ring_hi),
+                        min(N, ring_hi), max(1, ring_hi - 1), ring_hi})
+        sel = np.unique(np.concatenate([_ring_pixels(tb, rings), np.random.default_rng(ci).integers(0, o1, size=6000)]))
+        ref, _, _ = O.convolve(N, table, cfg.theta_max, inputs, sel=sel)
+        for b in range(B):
+            got = bout[b].cpu().numpy()
+            assert np.all(got[o1:] == -777.0)                        # nothing written beyond the cap
+            assert np.all(np.isfinite(got[:o1]))                     # nothing read beyond in_rows (NaN guard)
+            if exact:
+                omega64 = 4 * np.pi / cfg.npix
+                want = np.rint(ref[b] / omega64).astype(np.float32) * np.float32(omega64)
+                np.testing.assert_array_equal(got[sel], want)
+            else:
+                _check_values(got[sel], ref[b], f"cap cfg{ci} ring_hi {ring_hi}/{path}/map{b}")
+    with sc.Plan(N, T, cfg.theta_max, 1) as plan:
+        with pytest.raises(sc.ScError):
+            plan.cap_rows(0)
+        with pytest.raises(sc.ScError):
+            plan.cap_rows(2 * N + 1)
+
+
 def test_profile_entry_and_partition(sc):
     """sc_convolve_profile runs the same launches as sc_convolve (bit-identical output) and reports a
     positive device time for every kernel the plan uses; sc_plan_partition is consistent with them."""
