@@ -32,6 +32,10 @@ static __device__ __noinline__ unsigned belt_exact_mask(const Dev &P, int r, int
     const int N = P.nside, N4 = 4 * N;
     unsigned mask = 0;
     kq %= N4; if (kq < 0) kq += N4;
+    {   // one image decides for all unless it is within kImageMargin of the threshold
+        const double d0 = canonical_dot(P, r, k, rq, kq);
+        if (fabs(d0 - P.c) > fmax(kImageMargin, 2.0 * P.ke_band)) return d0 >= P.c ? 0xFFu : 0u;
+    }
     for (int h = 0; h < 2; ++h) {
         const int rp_i = h ? N4 - r : r, rq_i = h ? N4 - rq : rq;
         for (int m = 0; m < 4; ++m) {

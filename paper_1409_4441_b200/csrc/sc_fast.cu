@@ -41,9 +41,10 @@ struct HostGeo {
 // mirror: base pixels are the first half of the quadrant only, k = 0 .. (ip - 1 + sh) / 2 (the other half are their
 // reflections phi -> pi/2 - phi, computed by the same threads).
 // all_rings: also the base rings that the belt kernel normally takes (north-cap-only convolution).
+// lanes: lanes of a warp that own a group of R base pixels each (32; 16 in the lane-pair instance).
 static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, int r_hi, int r_lo, bool mirror,
-                           std::vector<SymTile> &tiles, bool all_rings = false) {
-    const int C = 32 * R;
+                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32) {
+    const int C = lanes * R;
     struct SubH { int r, k0, n, nw; int Lcap; double work; };
     auto make_sub = [&](int r, int k0, int n) {
         SubH sb{r, k0, n, (n + C - 1) / C, 0, 0.0};
@@ -102,6 +103,7 @@ static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, 
             tl.nsteps = std::max(tl.nsteps, tl.sub[i].ne);
             w0 += sb.nw; soff += sb.Lcap;
         }
+        tl.pad0 = soff;                                  // staged slots of the tile
     }
     return Lneed;
 }
@@ -115,6 +117,7 @@ struct FastCfg {            // per batch size
     bool tmem = false;            // 384-consumer variant with the running totals in tensor memory (large discs)
     bool tot = true;              // second accumulator set (per-ring partial sums added to running totals)
     bool mirror = false;          // 16 images per pair geometry (reflection phi -> pi/2 - phi as well)
+    bool pair = false;            // lane-pair instance: 16 lane pairs x R base pixels per warp
     std::map<std::pair<int, int>, std::pair<SymTile *, int>> band_tiles;   // (ring lo, hi) -> device tile list
     std::vector<int> ch_off, ch_lo, ch_hi;   // chunk i: tiles [ch_off[i], ch_off[i+1]), base rings ch_lo[i] .. ch_hi[i]
 };
@@ -148,7 +151,8 @@ struct FastPlan {
 static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, int B, cudaStream_t st,
                                 const SymTile *tiles, int nt, bool south = true) {
     if (nt <= 0) return cudaSuccess;
-    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south};
+    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair};
+    if (c.pair) return B == 1 ? dispatch_sym_pair(L, P, io, st) : cudaErrorInvalidValue;
     return B == 1 ? dispatch_sym_b1(L, P, io, st) : dispatch_sym_bn(L, P, io, B, st);
 }
 
@@ -197,7 +201,7 @@ cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, 
         auto it = c.band_tiles.find({s_lo, s_hi});
         if (it == c.band_tiles.end()) {
             std::vector<SymTile> tiles;
-            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, c.mirror, tiles);
+            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, c.mirror, tiles, false, c.pair ? 16 : 32);
             if (Lneed > c.Ltot) return cudaErrorInvalidValue;
             SymTile *d = nullptr;
             if ((e = cudaMalloc((void **)&d, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return e;
@@ -497,7 +501,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     // Tiles are packed from sub-tiles (runs of base pixels on one ring, 32 R pixels per warp): whole
     // CTA-wide runs first, the ragged remainders of all rings are bin-packed (first fit, decreasing).
     (void)max_batch;
-    struct Cand { int threads, R; bool mirror; };
+    struct Cand { int threads, R; bool mirror; bool pair = false; };
     for (int B = 1; B <= kMaxB; ++B) {
         FastCfg &c = fp->cfg[B];
         std::vector<Cand> cands;
@@ -513,21 +517,25 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         // one map per launch: 16 images per pair geometry (mirror symmetry as well) -- half the table gathers and
         // geometry per pair; twice the staged bytes per base pixel, so 192 consumer threads x 4 base pixels
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR")) cands.insert(cands.begin(), Cand{192, 4, true});
+        // ... and as lane pairs (sc_sym_pair.cu): 32 accumulators per lane, 12 (small discs) or 8 consumer warps
+        if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && std::getenv("SC_SYM_PAIR"))
+            cands.insert(cands.begin(), mean_nb <= 700.0 ? Cand{env_int("SC_PAIR_NC", 384), 4, true, true} : Cand{256, 4, true, true});
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
         if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256 || (ft == 384 && fr == 4 && B == 1)))
             cands.insert(cands.begin(), Cand{ft, fr, false});
         for (const Cand &cd : cands) {
-            const int R = cd.R, W = cd.threads / 32, C = 32 * R;
+            const int R = cd.R, W = cd.threads / 32, C = (cd.pair ? 16 : 32) * R;
             // full-width runs may be a little shorter than the CTA (last lanes idle) if that makes the
             // staged runs fit into shared memory
             for (int shrink = 0; shrink <= W * C / 4 && !c.ok; shrink += 16) {
             const int run = W * C - shrink;
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int npl = cd.mirror ? 4 : 2;                      // staged planes per position (float4 of rotation images each)
-            const int Lmax = (int)(((size_t)smem_optin - 256 - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
+            const size_t stat = cd.pair ? 3072 : 256;            // static shared memory of the kernel (barriers; step records)
+            const int Lmax = (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
             HostGeo &g = *fp->geo;
             g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;
-            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl); };
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32); };
             // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
             // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
             std::vector<SymTile> tiles;
@@ -550,13 +558,14 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
                 }
             }
             const size_t smem = tab_bytes + (size_t)kSymBufH * B * npl * Ltot * 16;
-            if (smem + 256 > (size_t)smem_optin) continue;        // 256: static shared memory (barriers)
+            if (smem + stat > (size_t)smem_optin) continue;
             c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
             c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all; c.run = run;
-            c.mirror = cd.mirror;
-            c.tmem = (B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb > 700.0);      // large discs: two-level sums, totals in TMEM
+            c.mirror = cd.mirror; c.pair = cd.pair;
+            c.tmem = !cd.pair && (B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb > 700.0);      // large discs: two-level sums, totals in TMEM
             // a single accumulator set (plain fp32 running sums) only for one map and discs of at most 700 pixels
             c.tot = !(B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb <= 700.0);
+            if (cd.pair) c.tot = mean_nb > 700.0;
             if ((e = cudaMalloc((void **)&c.tiles, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return fail(e);
             if (!tiles.empty() && (e = cudaMemcpy(c.tiles, tiles.data(), tiles.size() * sizeof(SymTile), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             c.ok = true;

@@ -52,7 +52,9 @@ struct SymLaunch {
     int threads, R;             // consumer threads, base pixels per thread
     size_t smem;
     bool tot, tmem, mirror, south;
+    bool pair;                  // lane-pair instance (sc_sym_pair.cu): two lanes share a group of R base pixels
 };
+cudaError_t dispatch_sym_pair(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
 cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
 cudaError_t dispatch_sym_bn(const SymLaunch &L, const Dev &P, const Maps &io, int B, cudaStream_t st);
 

@@ -103,6 +103,12 @@ __device__ __forceinline__ void zoned_cell(const Dev &P, float t, int &j, float 
     f = w - (float)i;
 }
 
+// The symmetric images of a pair (rotations by pi/2, z -> -z, the reflection phi -> pi/2 - phi) have the same z z' and
+// s s' bit for bit and azimuth differences that agree up to the rounding of phi0 + k dphi (a few 1e-16 rad), so their
+// canonical dots differ by less than 1e-14.  If one image is further than this from cos(theta_max), all images share its
+// verdict and need not be evaluated one by one (the guard band is ~3e-10 wide in these units: 1 pair in 30 goes on).
+constexpr double kImageMargin = 1e-11;
+
 // Exact decision for one pair (slow path).  If `au` is given the pair is also audited.
 static __device__ __noinline__ bool exact_included(const Dev &P, int rp, int kp, int rq, int kq, float t32,
                                             const Audit *au) {

@@ -53,6 +53,10 @@ static __device__ __noinline__ unsigned sym_exact_mask(const Dev &P, int r, int 
     const int n = 4 * ip, nq = 4 * ipq;
     unsigned mask = 0;
     kq %= nq; if (kq < 0) kq += nq;
+    {   // one image decides for all unless it is within kImageMargin of the threshold
+        const double d0 = canonical_dot(P, r, k, rq, kq);
+        if (fabs(d0 - P.c) > fmax(kImageMargin, 2.0 * P.ke_band)) return d0 >= P.c ? (1u << (4 * (1 + south) * (1 + mirror))) - 1u : 0u;
+    }
     int pl = 0;
     for (int mi = 0; mi <= mirror; ++mi) {
         // reflection phi -> pi/2 - phi: (2 k' + 1 - sh) = 2 ip - (2 k + 1 - sh)
