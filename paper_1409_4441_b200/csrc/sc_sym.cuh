@@ -502,7 +502,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 // i + 1 are issued before the FMAs of position i, the geometry of position i + 2 after them.  The
                 // number of positions is the same for all lanes (2 hw + R - 2 (R - 1) or 2 hw + R).
                 int left = plast - pos + 1;
-                constexpr bool PIPE = NC != 384;                     // 384 consumers: 152 registers per thread, no room
+                constexpr bool PIPE = NC == 192;                     // only the 6-warp instance needs it (elsewhere: spills, slower)
                 if (!PIPE) {
 #pragma unroll 2
                     for (; pos <= plast; ++pos) body(pos, ALL);
