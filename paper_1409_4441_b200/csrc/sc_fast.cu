@@ -145,13 +145,14 @@ struct FastPlan {
     std::shared_ptr<HostGeo> geo;
     int belt_tiles_per_ring = 0, belt_slack = 0;
     int *grp_off = nullptr, *grp_e = nullptr;
+    int *tile_ctr = nullptr;      // device counter of the sym kernel's dynamic tile schedule
 };
 
 // the sym kernel instance of this batch size over a tile list
 static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, int B, cudaStream_t st,
                                 const SymTile *tiles, int nt, bool south = true) {
     if (nt <= 0) return cudaSuccess;
-    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair};
+    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair, fp->tile_ctr};
     if (c.pair) return B == 1 ? dispatch_sym_pair(L, P, io, st) : cudaErrorInvalidValue;
     return B == 1 ? dispatch_sym_b1(L, P, io, st) : dispatch_sym_bn(L, P, io, B, st);
 }
@@ -306,7 +307,7 @@ void fast_plan_destroy(FastPlan *fp) {
         for (auto &kv : c.band_tiles) cudaFree(kv.second.first);
     }
     for (auto &kv : fp->caps) cudaFree(kv.second.tiles);
-    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->grp_off); cudaFree(fp->grp_e);
+    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->grp_off); cudaFree(fp->grp_e); cudaFree(fp->tile_ctr);
     delete fp;
 }
 
@@ -400,6 +401,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     cudaError_t e;
     if ((e = cudaMalloc((void **)&fp->pairs, std::max<size_t>(pairs.size(), 1) * sizeof(PairEnt))) != cudaSuccess) return fail(e);
     if ((e = cudaMalloc((void **)&fp->pair_off, pair_off.size() * sizeof(int))) != cudaSuccess) return fail(e);
+    if ((e = cudaMalloc((void **)&fp->tile_ctr, 64)) != cudaSuccess) return fail(e);
     if ((e = cudaMemcpy(fp->pairs, pairs.data(), pairs.size() * sizeof(PairEnt), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
     if ((e = cudaMemcpy(fp->pair_off, pair_off.data(), pair_off.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
 

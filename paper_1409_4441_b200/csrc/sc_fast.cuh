@@ -41,6 +41,7 @@ struct FastDev {
     int Ltot;               // staged positions per plane
     int ntab_s;             // entries of the shared-memory table
     int dbg;                // measurement only (SC_DBG): 1 = consumers skip the pair loop, 2 = producers skip the copies
+    int *tile_ctr;          // sym kernel: tile counter of the launch (zeroed before it): CTAs take tiles in list order as they finish
 };
 
 // What a launch of the sym kernel needs from the plan (host); the instantiations live in sc_sym_b1.cu (one map per
@@ -53,6 +54,7 @@ struct SymLaunch {
     size_t smem;
     bool tot, tmem, mirror, south;
     bool pair;                  // lane-pair instance (sc_sym_pair.cu): two lanes share a group of R base pixels
+    int *tile_ctr;              // plan-owned device counter for the dynamic tile schedule
 };
 cudaError_t dispatch_sym_pair(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
 cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);

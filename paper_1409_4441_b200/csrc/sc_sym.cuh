@@ -148,11 +148,10 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);
     const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 127) & ~(size_t)127));
     __shared__ unsigned long long full_bar[kSymBuf], empty_bar[kSymBuf];
+    __shared__ int s_tile[4];                            // tiles taken by this CTA (ring): written by producer 0, -1 = no more
     const int tid = threadIdx.x;
     const int N = P.nside;
     const int Ltot = F.Ltot;
-    const int GS = gridDim.x, bid = blockIdx.x;
-    const int nrows = (F.ntiles + GS - 1) / GS;
 
     for (int i = tid; i < F.ntab_s; i += blockDim.x) tab[i] = P.tabh[i];
     if (tid == 0) {
@@ -177,9 +176,17 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
         if (NC == 256 || NC == 384 || (NC == 192 && SC_L192 == 0)) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         const int pt = tid - PROD0;
         const int m = pt & 3;                            // quadrant image staged by this thread
-        for (int row = 0; row < nrows; ++row) {
-            const int tile = snake_tile(row, GS, bid);
-            if (tile >= F.ntiles) continue;
+        // Dynamic schedule: the tile list is sorted by decreasing work and a CTA takes the next tile when it is done with
+        // its last one (one atomicAdd per tile by producer 0, handed to the other threads through s_tile).
+        for (int n = 0;; ++n) {
+            if (pt == 0) { const int t = atomicAdd(F.tile_ctr, 1); s_tile[n & 3] = t < F.ntiles ? t : -1; }
+            asm volatile("bar.sync 1, %0;" ::"n"(NPROD) : "memory");
+            const int tile = *(volatile int *)&s_tile[n & 3];
+            if (tile < 0) {                              // no more tiles: wake the consumers with one empty step
+                mbar_wait_sleep(&empty_bar[it % kSymBuf], ((it / kSymBuf) & 1u) ^ 1u);
+                cp_async_mbar_arrive(&full_bar[it % kSymBuf]);
+                break;
+            }
             const SymTile *tl = F.tiles + tile;
             const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
             for (int step = 0; step < nsteps; ++step, ++it) {
@@ -285,9 +292,11 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     unsigned tab_sh = smem_u32(tab) - kMagicBits * 8u;
     asm volatile("mov.u32 %0, %0;" : "+r"(tab_sh));
 
-    for (int row = 0; row < nrows; ++row) {
-        const int tile = snake_tile(row, GS, bid);
-        if (tile >= F.ntiles) continue;
+    for (int n = 0;; ++n) {
+        // the tile's number is valid once the producers have filled (arrived on) the buffer of its first step
+        mbar_wait(&full_bar[it % kSymBuf], (it / kSymBuf) & 1u);
+        const int tile = *(volatile int *)&s_tile[n & 3];
+        if (tile < 0) break;
         const SymTile *tl = F.tiles + tile;
         const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
         int si = 0;
@@ -612,12 +621,13 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
 template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
 static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st) {
     const char *dbg = std::getenv("SC_DBG");
-    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0};
+    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0, L.tile_ctr};
     static bool attr_done[64] = {};
     cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = std::min(L.nsm, L.ntiles);
     if (grid <= 0) return cudaSuccess;
+    if ((e = cudaMemsetAsync(L.tile_ctr, 0, sizeof(int), st)) != cudaSuccess) return e;      // the launch's tile counter
     sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
