@@ -622,29 +622,43 @@ sc_status sc_band_partition(const sc_plan *plan, int world, int rank, int *ring_
     if (!plan) return SC_ERR_INVALID_ARG;
     const int N = plan->dev.nside;
     if (world < 1 || world > 2 * N || rank < 0 || rank >= world) return SC_ERR_INVALID_ARG;
-    // base ring r stands for rings r and 4N - r: 2 n_r pixels (n_r for the equator ring 2N).  Bands get
-    // nearly equal ESTIMATED WORK: a cap pixel (sym kernel) costs about 3.3 belt pixels (stencil) and a pixel
-    // next to the poles (warp-per-pixel kernel) about 65 (measured ratios, configs 4 and 5).
+    // base ring r stands for rings r and 4N - r: 2 n_r pixels (n_r for the equator ring 2N).  Bands get nearly equal
+    // ESTIMATED TIME from per-pixel costs measured on one B200 (configs 4 and 5, round 2): with nb neighbours per pixel a
+    // belt pixel costs ~5.3e-11 nb ms, a cap pixel 2.9 times that, a pixel next to the poles (warp-per-pixel kernel)
+    // 6.8e-6 + 2.9e-9 nb ms, i.e. 55 + 128000 / nb belt pixels (356 at config 4, 88 at config 5).  A band boundary that
+    // falls close to a hand-over between two kernels is moved onto it, so that no band pays a kernel launch (prologue:
+    // the 128 KB table per CTA) for a sliver of rings.
     const int pr = plan->fast ? plan->polar_rings : 0;
     const int fb = plan->fast ? sc::fast_first_belt_ring(plan->fast) : 2 * N + 1;
+    const double nb = std::max(1.0, 0.5 * (double)plan->dev.npix * ((double)plan->dev.tmax / plan->dev.scale));
+    const int64_t w_polar = (int64_t)(10.0 * (55.0 + 128000.0 / nb));            // in tenths of a belt pixel
     auto weight = [&](int r) -> int64_t {
         const int64_t px = (int64_t)plan->rings[r - 1].n * (r < 2 * N ? 2 : 1);
-        return px * (r <= pr ? 200 : (r < fb ? 10 : 3));
+        return px * (r <= pr ? w_polar : (r < fb ? 29 : 10));
     };
     int64_t total = 0;
     for (int r = 1; r <= 2 * N; ++r) total += weight(r);
-    auto first_ring = [&](int k) -> int {            // first base ring of band k (band `world` starts at 2N + 1)
-        if (k <= 0) return 1;
-        if (k >= world) return 2 * N + 1;
+    std::vector<int> first(world + 1, 1);            // first base ring of band k; band `world` starts at 2N + 1
+    first[world] = 2 * N + 1;
+    {
         int64_t cum = 0;
         int r = 1;
-        for (; r <= 2 * N; ++r) {
-            if (cum * world >= total * k) break;
-            cum += weight(r);
+        for (int k = 1; k < world; ++k) {
+            for (; r <= 2 * N; ++r) {
+                if (cum * world >= total * k) break;
+                cum += weight(r);
+            }
+            first[k] = r;
         }
-        // every band keeps at least one ring
-        return std::min(std::max(r, k + 1), 2 * N - (world - 1 - k));
-    };
+        const int snap = std::max(2, N / 16);
+        for (int k = 1; k < world; ++k) {
+            if (pr > 0 && std::abs(first[k] - (pr + 1)) <= snap) first[k] = pr + 1;
+            if (fb <= 2 * N && std::abs(first[k] - fb) <= snap) first[k] = fb;
+        }
+        for (int k = 1; k < world; ++k)              // every band keeps at least one ring
+            first[k] = std::min(std::max(first[k], std::max(k + 1, first[k - 1] + 1)), 2 * N - (world - 1 - k));
+    }
+    auto first_ring = [&](int k) -> int { return first[std::min(std::max(k, 0), world)]; };
     const int lo = first_ring(rank), hi = first_ring(rank + 1) - 1;
     if (hi < lo) return SC_ERR_INVALID_ARG;
     if (ring_lo) *ring_lo = lo;
