@@ -499,6 +499,29 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         }
     }
 
+    // ---- step order of the sym kernel: a step's pair loop takes time ~ the ring's half window, its staging a constant
+    // (the whole run), so the rings at the edge of the disc are short steps in which the consumers outrun the producers.
+    // Alternate long and short steps (the two stage buffers then average over a pair) instead of walking the rings from
+    // north to south.  Belt rings keep their order (tap groups of the belt kernel).
+    if (!std::getenv("SC_SYM_RINGORDER")) {
+        for (int r = polar + 1; r <= 2 * N; ++r) {
+            if (is_belt[r]) continue;
+            std::vector<PairEnt> &lst = per_ring[r];
+            std::vector<int> idx(lst.size());
+            for (size_t i = 0; i < idx.size(); ++i) idx[i] = (int)i;
+            std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return lst[a].hw > lst[b].hw; });
+            std::vector<PairEnt> out;
+            out.reserve(lst.size());
+            for (size_t lo = 0, hi = idx.size(); lo < hi;) {
+                out.push_back(lst[idx[lo++]]);
+                if (lo < hi) out.push_back(lst[idx[--hi]]);
+            }
+            lst = out;
+            std::copy(lst.begin(), lst.end(), pairs.begin() + pair_off[slot_of[r]]);
+        }
+        if ((e = cudaMemcpy(fp->pairs, pairs.data(), pairs.size() * sizeof(PairEnt), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+    }
+
     // ---- sym kernel: per batch size pick (threads, R) so that table + double-buffered stage fit ------
     // Tiles are packed from sub-tiles (runs of base pixels on one ring, 32 R pixels per warp): whole
     // CTA-wide runs first, the ragged remainders of all rings are bin-packed (first fit, decreasing).
