@@ -237,6 +237,18 @@ sc_status sc_debug_fma_peak(int packed, double *fma_per_s, double *elapsed_ms);
 /* Kernel launches enqueued by the last sc_convolve / sc_convolve_host on this plan. */
 int sc_last_launch_count(const sc_plan *plan);
 
+/*
+ * sc_plan_double_coordinate -- 1 if the plan's kernels form the table coordinate t = (1 - cos theta_pq) (n-1)/(1-c) of every
+ * pair in fp64 (and split it into table cell + position in the cell), 0 if in fp32.  Chosen at plan creation from the
+ * table alone: fp32 resolves t to ~t 2^-23 cells, i.e. K to |slope of cell j| j 2^-23; if that, rms over the cells,
+ * exceeds 6.5e-7 of the table's rms -- oscillating tables such as the real-space part of the paper's least-squares
+ * split (Fig. 4) at theta_cut of degrees -- fp32 geometry alone would break the 1e-6 bar (DESIGN.md
+ * section 10; the paper reports this single-precision sensitivity as alpha = 5).  Such plans run one map
+ * per launch through the 16-image sym instance, the belt stencil (taps in fp64) and the generic kernels; the two-zone
+ * table is not combined with it.  Products and sums stay fp32.  NULL plan: 0.
+ */
+int sc_plan_double_coordinate(const sc_plan *plan);
+
 const char *sc_status_string(sc_status s);
 /* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
 const char *sc_last_cuda_error(void);

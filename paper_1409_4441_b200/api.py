@@ -16,7 +16,7 @@ KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
 EXPORTS = ("sc_plan_create", "sc_plan_create_zoned", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
            "sc_band_partition", "sc_convolve_band", "sc_cap_rows", "sc_convolve_cap",
            "sc_plan_destroy", "sc_plan_set_path",
-           "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_debug_fma_peak", "sc_last_launch_count",
+           "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_debug_fma_peak", "sc_last_launch_count", "sc_plan_double_coordinate",
            "sc_status_string", "sc_last_cuda_error", "sc_version")
 
 _lib = None
@@ -56,6 +56,7 @@ def lib():
         l.sc_debug_neighbour_counts.argtypes = [vp, vp, vp, vp]
         l.sc_debug_stats.argtypes = [vp, vp, vp, vp]
         l.sc_last_launch_count.argtypes = [vp]
+        l.sc_plan_double_coordinate.argtypes = [vp]
         l.sc_debug_fma_peak.argtypes = [i32, vp, vp]
         for f in ("sc_status_string", "sc_last_cuda_error", "sc_version"):
             getattr(l, f).restype = C.c_char_p
@@ -196,6 +197,10 @@ def sc_last_launch_count(plan):
     return lib().sc_last_launch_count(plan)
 
 
+def sc_plan_double_coordinate(plan):
+    return lib().sc_plan_double_coordinate(plan)
+
+
 class Plan:
     """Convenience owner of a plan for torch users: maps are torch CUDA fp32 tensors."""
 
@@ -223,6 +228,7 @@ class Plan:
     def info(self):
         d = sc_plan_info(self.handle)
         d.update(sc_debug_stats(self.handle))
+        d["double_coordinate"] = sc_plan_double_coordinate(self.handle)
         return d
 
     def set_path(self, path):

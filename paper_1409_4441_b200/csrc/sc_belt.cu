@@ -50,7 +50,10 @@ static __device__ __noinline__ unsigned belt_exact_mask(const Dev &P, int r, int
 // One stencil tap: weight of the pair at azimuthal pixel offset j (same arithmetic as the sym kernel).
 // Returns the weight (0 if excluded or uncertain); `unc` is set for taps inside the guard band, whose
 // inclusion is decided per pixel pair in fp64 later; Ku is the weight such a pair gets if included.
-__device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j, float dcc, bool &unc, float &Ku) {
+// pd: the ring pair in fp64 for plans with the fp64 table coordinate (Dev::hp; dcc64 = offset to the nearest pixel), else
+// unused.
+__device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j, float dcc, bool &unc, float &Ku,
+                                          const PairEntD *pd = nullptr, double dcc64 = 0.0) {
     const float d = fmaf((float)j, pe.dphi, dcc);
     const float y = d * d;
     float h = fmaf(y, pe.c4, pe.c3);
@@ -67,6 +70,7 @@ __device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j
                 unc = true;
                 float xk = fminf(t, P.tmax) - 0.5f;
                 if (P.zoned) { int jz; zoned_cell(P, fminf(t, P.tmax), jz, xk); xk -= 0.5f; }   // last cell, centred form
+                if (P.hp) xk = fminf(t, P.tmax) - (float)(P.ntab - 2) - 0.5f;                   // cell-local table
                 Ku = fmaf(xk, el.y, el.x);
             }
             return 0.f;
@@ -77,6 +81,13 @@ __device__ __forceinline__ float belt_tap(const Dev &P, const PairEnt &pe, int j
         zoned_cell(P, tp + 0.5f, jz, fz);
         const float2 el = __ldg(&P.tabh[jz]);
         return fmaf(fz - 0.5f, el.y, el.x);
+    }
+    if (P.hp) {                                      // fp64 coordinate -> cell + position in the cell (t < tmax - eps here)
+        if (!pd) return 0.f;                         // (rescan of the uncertain taps: the weight is not used)
+        const double t64 = fma(pd->Bs, one_minus_cos_poly_f64(fma((double)j, pd->dphi, dcc64)), pd->A);
+        const int cell = min(__double2int_rd(t64), P.ntab - 2);
+        const float2 el = __ldg(&P.tabh[cell]);
+        return fmaf((float)(t64 - (double)cell) - 0.5f, el.y, el.x);
     }
     const float2 el = __ldg(&P.tabh[bits - kMagicBits]);
     return fmaf(tp, el.y, el.x);
@@ -201,6 +212,9 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     // Y = N (2k + 1 - sh + shq), so delta = (1 - sh + shq) >> 1 and the remainder is N or 0.
                     const int Yk = 1 - sh + pe.shq;
                     const float dcc = (float)(N - ((Yk & 1) ? N : 0)) * pe.cdc;
+                    PairEntD pd{};
+                    if (P.hp) pd = F.pairsd[e0 + e];
+                    const double dcc64 = (double)(N - ((Yk & 1) ? N : 0)) * pd.cdc;
                     // S[i] = (w[x], w[x-1]), x = i - 2 - a0: chunk g of 4 staged positions uses S[4g .. 4g+5]
                     const int nS = 4 * ng + 2;
                     for (int i = pt; i < nS; i += kTapThreads) {
@@ -212,7 +226,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                             float w = 0.f;
                             if (xx >= 0 && xx <= 2 * pe.hw) {
                                 bool unc; float Ku;
-                                w = belt_tap(P, pe, xx - pe.hw, dcc, unc, Ku);
+                                w = belt_tap(P, pe, xx - pe.hw, dcc, unc, Ku, &pd, dcc64);
                                 if (unc && q == 0) {                          // list every uncertain tap once
                                     const int slot = atomicAdd(nexc, 1);
                                     if (slot < kMaxExc) { exc_e[slot] = e; exc_j[slot] = xx - pe.hw; exc_k[slot] = Ku; }
@@ -409,7 +423,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                         const float dcc = (float)(N - ((Yk & 1) ? N : 0)) * pe.cdc;
                         for (int j = -pe.hw; j <= pe.hw; ++j) {
                             bool unc; float Ku;
-                            belt_tap(P, pe, j, dcc, unc, Ku);
+                            belt_tap(P, pe, j, dcc, unc, Ku);                     // (only `unc` and Ku are used: no fp64 needed)
                             if (unc) apply(pe, j, Ku);
                         }
                     }

@@ -146,13 +146,14 @@ struct FastPlan {
     int belt_tiles_per_ring = 0, belt_slack = 0;
     int *grp_off = nullptr, *grp_e = nullptr;
     int *tile_ctr = nullptr;      // device counter of the sym kernel's dynamic tile schedule
+    PairEntD *pairsd = nullptr;   // fp64 ring pairs (Dev::hp plans)
 };
 
 // the sym kernel instance of this batch size over a tile list
 static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, int B, cudaStream_t st,
                                 const SymTile *tiles, int nt, bool south = true) {
     if (nt <= 0) return cudaSuccess;
-    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair, fp->tile_ctr};
+    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair, fp->tile_ctr, fp->pairsd};
     if (c.pair) return B == 1 ? dispatch_sym_pair(L, P, io, st) : cudaErrorInvalidValue;
     return B == 1 ? dispatch_sym_b1(L, P, io, st) : dispatch_sym_bn(L, P, io, B, st);
 }
@@ -307,7 +308,7 @@ void fast_plan_destroy(FastPlan *fp) {
         for (auto &kv : c.band_tiles) cudaFree(kv.second.first);
     }
     for (auto &kv : fp->caps) cudaFree(kv.second.tiles);
-    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->grp_off); cudaFree(fp->grp_e); cudaFree(fp->tile_ctr);
+    cudaFree(fp->woff); cudaFree(fp->belt_tiles); cudaFree(fp->grp_off); cudaFree(fp->grp_e); cudaFree(fp->tile_ctr); cudaFree(fp->pairsd);
     delete fp;
 }
 
@@ -474,7 +475,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((e = cudaMemcpy(fp->grp_off, grp_off.data(), grp_off.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             if ((e = cudaMalloc((void **)&fp->grp_e, grp_e.size() * sizeof(int))) != cudaSuccess) return fail(e);
             if ((e = cudaMemcpy(fp->grp_e, grp_e.data(), grp_e.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
-            fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, fp->grp_off, fp->grp_e, (int)btiles.size(), pw_max, ne_max, nbuf, ntb};
+            fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, fp->grp_off, fp->grp_e, (int)btiles.size(), pw_max, ne_max, nbuf, ntb, nullptr};
             fp->belt_slack = bv.slack;
             fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true; fp->belt_tiles_per_ring = N / T;
             // latitude chunks: the tile list runs from ring 2N down to the first belt ring, N / T tiles per ring
@@ -522,6 +523,24 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         if ((e = cudaMemcpy(fp->pairs, pairs.data(), pairs.size() * sizeof(PairEnt), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
     }
 
+    // ---- fp64 ring pairs for plans with steep tables (Dev::hp), in the final order of `pairs` ------------------------
+    if (P.hp) {
+        std::vector<PairEntD> pd(pairs.size());
+        for (int r = polar + 1; r <= 2 * N; ++r) {
+            const int base = pair_off[slot_of[r]];
+            for (size_t i = 0; i < per_ring[r].size(); ++i) {
+                const int rq = per_ring[r][i].rq;
+                double A64 = 1.0 - (z[r - 1] * z[rq - 1] + s[r - 1] * s[rq - 1]);
+                if (A64 < 0) A64 = 0;
+                pd[base + i] = PairEntD{A64 * P.scale, s[r - 1] * s[rq - 1] * P.scale, 2.0 * M_PI / (4.0 * ipof(rq)),
+                                        M_PI / (4.0 * (double)ipof(r) * (double)ipof(rq))};
+            }
+        }
+        if ((e = cudaMalloc((void **)&fp->pairsd, std::max<size_t>(pd.size(), 1) * sizeof(PairEntD))) != cudaSuccess) return fail(e);
+        if ((e = cudaMemcpy(fp->pairsd, pd.data(), pd.size() * sizeof(PairEntD), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
+        if (fp->belt_ok) fp->belt.pairsd = fp->pairsd;
+    }
+
     // ---- sym kernel: per batch size pick (threads, R) so that table + double-buffered stage fit ------
     // Tiles are packed from sub-tiles (runs of base pixels on one ring, 32 R pixels per warp): whole
     // CTA-wide runs first, the ragged remainders of all rings are bin-packed (first fit, decreasing).
@@ -545,8 +564,12 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         // ... and as lane pairs (sc_sym_pair.cu): 32 accumulators per lane, 12 (small discs) or 8 consumer warps
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && std::getenv("SC_SYM_PAIR"))
             cands.insert(cands.begin(), mean_nb <= 700.0 ? Cand{env_int("SC_PAIR_NC", 384), 4, true, true} : Cand{256, 4, true, true});
+        if (P.hp) {                                         // fp64 table coordinate: the 16-image instance only, one map per launch
+            if (B > 1) continue;
+            cands = {Cand{192, 4, true}, Cand{256, 4, false}, Cand{256, 2, false}, Cand{128, 2, false}};
+        }
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
-        if (fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256 || (ft == 384 && fr == 4 && B == 1)))
+        if (!P.hp && fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256 || (ft == 384 && fr == 4 && B == 1)))
             cands.insert(cands.begin(), Cand{ft, fr, false});
         for (const Cand &cd : cands) {
             const int R = cd.R, W = cd.threads / 32, C = (cd.pair ? 16 : 32) * R;

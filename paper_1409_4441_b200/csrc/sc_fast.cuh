@@ -19,6 +19,9 @@ struct PairEnt {            // uniform per (base ring, input ring); 56 bytes
     int pad_;
 };
 
+// The same ring pair in fp64 for plans with Dev::hp (steep tables): t = A + Bs (1 - cos d), d = (integer offset) cdc + j dphi
+struct PairEntD { double A, Bs, dphi, cdc; };
+
 // A tile of the sym kernel is a set of up to kMaxSub sub-tiles, each a run of base pixels on one ring that
 // is worked on by `nw` consecutive warps (32 R pixels per warp).  Packing several short runs into one
 // tile keeps all warps of the CTA busy on the short rings of the polar caps.
@@ -41,6 +44,7 @@ struct FastDev {
     int Ltot;               // staged positions per plane
     int ntab_s;             // entries of the shared-memory table
     int dbg;                // measurement only (SC_DBG): 1 = consumers skip the pair loop, 2 = producers skip the copies
+    const PairEntD *pairsd; // fp64 ring pairs (Dev::hp), same index as pairs; else nullptr
     int *tile_ctr;          // sym kernel: tile counter of the launch (zeroed before it): CTAs take tiles in list order as they finish
 };
 
@@ -55,6 +59,7 @@ struct SymLaunch {
     bool tot, tmem, mirror, south;
     bool pair;                  // lane-pair instance (sc_sym_pair.cu): two lanes share a group of R base pixels
     int *tile_ctr;              // plan-owned device counter for the dynamic tile schedule
+    const PairEntD *pairsd;     // fp64 ring pairs of a Dev::hp plan
 };
 cudaError_t dispatch_sym_pair(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
 cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
@@ -74,6 +79,7 @@ struct BeltDev {
     int ne_max;               // input rings per group, at most
     int nbuf;                 // stage buffers
     int ntb;                  // tap buffers (1 or 2)
+    const PairEntD *pairsd;   // fp64 ring pairs (Dev::hp), same index as pairs; else nullptr
 };
 
 // Layout of one tap buffer in shared memory (bytes): taps | ring descriptors | exception list

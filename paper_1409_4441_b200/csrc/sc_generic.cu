@@ -58,7 +58,8 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
             // nearest pixel of ring rq in azimuth and the (small) offset to it
             const double xq = (phip - P.phi0[rq - 1]) / dphiq;
             int kc = (int)rint(xq);
-            const float dc = (float)((P.phi0[rq - 1] + (double)kc * dphiq) - phip);
+            const double dc64 = (P.phi0[rq - 1] + (double)kc * dphiq) - phip;
+            const float dc = (float)dc64;
             kc %= nq; if (kc < 0) kc += nq;
             int jlo, jcnt;
             if (wmax >= 2.f) { jlo = -(nq / 2); jcnt = nq; }
@@ -92,6 +93,11 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
                         int i = (int)tt;
                         float xk = tt;                                  // K = tab[i].x + xk tab[i].y
                         if (P.zoned) zoned_cell(P, tt, i, xk);
+                        else if (P.hp) {                                // fp64 coordinate -> cell + position in the cell
+                            const double t64 = fmin(fma(sp * sq * P.scale, one_minus_cos_f64(fma((double)j, dphiq, dc64)), A64 * P.scale), (double)P.tmax);
+                            i = min((int)t64, P.ntab - 2);
+                            xk = (float)(t64 - (double)i);
+                        }
                         else if (i > P.ntab - 2) i = P.ntab - 2;
                         const float2 e = __ldg(&P.tab[i]);
                         const float K = fmaf(xk, e.y, e.x);
@@ -161,7 +167,8 @@ generic_warp_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1) 
         const float dphiq_f = (float)dphiq;
         const double xq = (phip - P.phi0[rq - 1]) / dphiq;
         int kc = (int)rint(xq);
-        const float dc = (float)((P.phi0[rq - 1] + (double)kc * dphiq) - phip);
+        const double dc64 = (P.phi0[rq - 1] + (double)kc * dphiq) - phip;
+        const float dc = (float)dc64;
         kc %= nq; if (kc < 0) kc += nq;
         int jlo, jcnt;
         if (wmax >= 2.f) { jlo = -(nq / 2); jcnt = nq; }
@@ -192,6 +199,11 @@ generic_warp_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1) 
                 int i = (int)tt;
                 float xk = tt;                                  // K = tab[i].x + xk tab[i].y
                 if (P.zoned) zoned_cell(P, tt, i, xk);
+                else if (P.hp) {                                // fp64 coordinate -> cell + position in the cell
+                    const double t64 = fmin(fma(sp * sq * P.scale, one_minus_cos_f64(fma((double)j, dphiq, dc64)), A64 * P.scale), (double)P.tmax);
+                    i = min((int)t64, P.ntab - 2);
+                    xk = (float)(t64 - (double)i);
+                }
                 else if (i > P.ntab - 2) i = P.ntab - 2;
                 const float2 e = __ldg(&P.tab[i]);
                 const float K = fmaf(xk, e.y, e.x);

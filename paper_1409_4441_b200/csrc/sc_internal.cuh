@@ -36,7 +36,29 @@ struct Dev {
     // two-zone table (R11): the lookup coordinate is tau = min(z_alpha t, z_beta + z_gamma t), t = (1-dot) scale
     int zoned, z_hm1;                     // z_hm1 = n/2 - 1: cells of the inner zone
     float z_alpha, z_gamma, z_t1g;        // inner zone: tau = z_alpha t; outer zone: tau = z_hm1 + z_gamma t - z_t1g
+    // steep tables: the table coordinate of every pair is formed in fp64
+    // and split into cell + position in the cell; the tables are then in the cell-local form of the two-zone mode
+    int hp;
 };
+
+// 1 - cos d for |d| <= pi in fp64: 2 sin^2(d/2) (generic kernels, any azimuth difference)
+__device__ __forceinline__ double one_minus_cos_f64(double d) {
+    const double sh = sin(0.5 * d);
+    return 2.0 * sh * sh;
+}
+// ... and for |d| <= 0.9 rad by its even series through d^16 (next term < 1e-14 relative): the fast kernels
+__device__ __forceinline__ double one_minus_cos_poly_f64(double d) {
+    const double y = d * d;
+    double p = -1.0 / 20922789888000.0;                  // 16!
+    p = fma(y, p, 1.0 / 87178291200.0);                  // 14!
+    p = fma(y, p, -1.0 / 479001600.0);                   // 12!
+    p = fma(y, p, 1.0 / 3628800.0);                      // 10!
+    p = fma(y, p, -1.0 / 40320.0);
+    p = fma(y, p, 1.0 / 720.0);
+    p = fma(y, p, -1.0 / 24.0);
+    p = fma(y, p, 0.5);
+    return y * p;
+}
 
 // Audit outputs (plan creation / debug only)
 struct Audit {

@@ -265,6 +265,20 @@ sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const do
             if (!(alpha >= gamma)) { st = SC_ERR_INVALID_ARG; break; }
             D.zoned = 1; D.z_hm1 = h - 1; D.z_alpha = (float)alpha; D.z_gamma = (float)gamma; D.z_t1g = (float)(t1 * gamma);
         }
+        // Steep tables: the fp32 pair geometry resolves the table coordinate to ~t 2^-23 cells, i.e. the kernel to
+        // |b_j| j 2^-23 in cell j (b_j = cell slope).  If that, rms over the cells (pairs are uniform in t), exceeds 6.5e-7
+        // of the table's rms, the kernels form the coordinate in fp64 (Dev::hp).  Not combined with the two-zone table.
+        D.hp = 0;
+        if (zone_frac == 0.0) {
+            double se = 0.0, sk = 0.0;
+            for (int j = 0; j + 1 < n_table; ++j) {
+                const double t0 = ktable[n_table - 1 - j], t1 = ktable[n_table - 2 - j];
+                const double err = (t1 - t0) * ((double)j + 0.5) * std::ldexp(1.0, -23);
+                se += err * err; sk += 0.25 * (t0 + t1) * (t0 + t1);
+            }
+            if (sk > 0.0 && std::sqrt(se / sk) > 6.5e-7) D.hp = 1;      // leaves 3.5e-7 of the 1e-6 bar to the fp32 accumulation
+            if (const char *e = std::getenv("SC_HP")) D.hp = std::atoi(e) != 0;
+        }
         if (const char *e = std::getenv("SC_KNIFE_EDGE_BAND")) { const double v = std::atof(e); if (v > 0) D.ke_band = v; }
 
         // ring tables
@@ -299,8 +313,8 @@ sc_status sc_plan_create_zoned(sc_plan **plan, int nside, int ordering, const do
             const double b = t1 - t0, a = t0 - (double)j * b;
             tab[j] = make_float2((float)a, (float)b);
             tabh[j] = make_float2((float)(a + 0.5 * b), (float)b);
-            if (zone_frac > 0.0) {
-                // two-zone table: cell-local form K = T_j + (tau - j) b_j (the cells of the outer zone carry
+            if (zone_frac > 0.0 || D.hp) {
+                // two-zone table / fp64 coordinate: cell-local form K = T_j + (tau - j) b_j (the cells of the outer zone carry
                 // twice the slope at twice the index: the intercept form would lose a digit to cancellation)
                 tab[j] = make_float2((float)t0, (float)b);
                 tabh[j] = make_float2((float)(t0 + 0.5 * b), (float)b);      // around the cell centre
@@ -380,6 +394,8 @@ sc_status sc_debug_stats(const sc_plan *plan, int64_t *n_uncertain, double *max_
 
 int sc_last_launch_count(const sc_plan *plan) { return plan ? plan->last_launches : 0; }
 
+int sc_plan_double_coordinate(const sc_plan *plan) { return plan ? plan->dev.hp : 0; }
+
 // Maps are N_pix floats each: no output may overlap an input or another output.
 static bool maps_ok(const float *const *in_maps, float *const *out_maps, int B, size_t npix) {
     const uintptr_t bytes = (uintptr_t)npix * 4;
@@ -410,7 +426,8 @@ static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps,
     int launches = 0;
     const size_t npix = (size_t)D.npix;
     // maps per launch; a NESTED plan goes through its RING work buffers, which hold nest_maps maps
-    const int chunk = plan->nested ? plan->nest_maps : sc::kMaxB;
+    // (plans with the fp64 table coordinate, Dev::hp, have one-map kernel instances only)
+    const int chunk = D.hp ? 1 : (plan->nested ? plan->nest_maps : sc::kMaxB);
     for (int b0 = 0; b0 < B; b0 += chunk) {
         const int nb = std::min(chunk, B - b0);
         sc::Maps io{};
@@ -499,7 +516,7 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
     if (!plan->own_stream) SC_CUDA(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
     const sc::Dev &D = plan->dev;
     const int N = D.nside;
-    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && !plan->nested && sc::fast_available(plan->fast, std::min(B, sc::kMaxB));
+    const bool pipelined = plan->path == SC_PATH_AUTO && plan->fast && !plan->nested && sc::fast_available(plan->fast, plan->dev.hp ? 1 : std::min(B, sc::kMaxB));
     if (!pipelined) {
         std::vector<const float *> in(B); std::vector<float *> out(B);
         for (int b = 0; b < B; ++b) {
@@ -538,8 +555,9 @@ sc_status sc_convolve_host(sc_plan *plan, const float *const *in_maps_host, floa
         *ev = plan->events[nev++];
         return SC_OK;
     };
-    for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
-        const int nb = std::min(sc::kMaxB, B - b0);
+    const int per_launch = D.hp ? 1 : sc::kMaxB;
+    for (int b0 = 0; b0 < B; b0 += per_launch) {
+        const int nb = std::min(per_launch, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = plan->stage_in + npix * (b0 + b); io.out[b] = plan->stage_out + npix * (b0 + b); }
         auto copy_in = [&](size_t p0, size_t p1) -> sc_status {
@@ -679,8 +697,9 @@ sc_status sc_convolve_band(sc_plan *plan, int ring_lo, int ring_hi, const float 
     int64_t orow[4];
     band_rows(plan, ring_lo, ring_hi, orow, nullptr);
     int launches = 0;
-    for (int b0 = 0; b0 < B; b0 += sc::kMaxB) {
-        const int nb = std::min(sc::kMaxB, B - b0);
+    const int per_launch = D.hp ? 1 : sc::kMaxB;
+    for (int b0 = 0; b0 < B; b0 += per_launch) {
+        const int nb = std::min(per_launch, B - b0);
         sc::Maps io{};
         for (int b = 0; b < nb; ++b) { io.in[b] = in_maps[b0 + b]; io.out[b] = out_maps[b0 + b]; }
         if (plan->path == SC_PATH_GENERIC || !sc::fast_available(plan->fast, nb)) {
@@ -740,7 +759,7 @@ sc_status sc_convolve_cap(sc_plan *plan, int ring_hi, const float *const *in_map
     for (int b = 0; b < B; ++b) {                                      // one map per launch (north-only kernel instance)
         sc::Maps io{};
         io.in[0] = in_maps[b]; io.out[0] = out_maps[b];
-        if (plan->path == SC_PATH_GENERIC || !plan->fast) {
+        if (plan->path == SC_PATH_GENERIC || !plan->fast || D.hp) {      // (no north-only instance with the fp64 coordinate)
             SC_CUDA(sc::launch_generic_conv(D, io, 1, 0, (int)orow[1], 0, 0, st));
             ++launches;
             continue;

@@ -135,9 +135,11 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 // TOT: per-step partial sums are added to a second accumulator set (pairwise-like summation; needed for
 // discs of thousands of pixels, costs as many registers again).
 // Z: two-zone table (lookup at tau(t), R11).  TM: the second accumulator set lives in tensor memory.
-template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
+// HP: table coordinate in fp64 (Dev::hp, steep tables), split into cell + position in the cell; cell-local table.
+template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR, bool HP = false>
 __global__ void __launch_bounds__(sym_threads(NC), 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
+    static_assert(!(HP && Z), "the fp64 coordinate is not combined with the two-zone table");
     static_assert(R == 1 || R == 2 || R == 4, "R");
     constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
     constexpr int NPROD = sym_nprod(NC), PROD0 = sym_prod0(NC);
@@ -349,6 +351,14 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 float dcr[R];
 #pragma unroll
                 for (int rr = 0; rr < R; ++rr) dcr[rr] = (float)(ip - rem - 2 * rr * pe.ipq) * pe.cdc;
+                // fp64 coordinate (HP): the same ring pair in double
+                PairEntD pd{};
+                double dcr64[HP ? R : 1], jd = -(double)pe.hw;
+                if (HP) {
+                    pd = F.pairsd[me.e0 + step];
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr) dcr64[rr] = (double)(ip - rem - 2 * rr * pe.ipq) * pd.cdc;
+                }
                 // staged position of input pixel kc + j: i0 + j (slot_of_pos: padded against bank conflicts)
                 const int i0 = kc - w0;
                 unsigned pn[B];                          // shared address of this sub-tile's first plane, map b
@@ -370,6 +380,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                                 const float2 el = tab[P.ntab - 2];
                                 float xk = fminf(t, tmax) - 0.5f;
                                 if (Z) { int jz; zoned_cell(P, fminf(t, tmax), jz, xk); xk -= 0.5f; }   // last cell, centred form
+                                if (HP) xk = fminf(t, tmax) - (float)(P.ntab - 2) - 0.5f;               // cell-local table
                                 const float Ku = fmaf(xk, el.y, el.x);
 #pragma unroll
                                 for (int b = 0; b < B; ++b) {
@@ -442,6 +453,20 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                             gt[2 * h] = fz.x; gt[2 * h + 1] = fz.y;
                             gc[2 * h] = __float_as_uint(bz.x) + (o0 ? zhm1 : 0u); gc[2 * h + 1] = __float_as_uint(bz.y) + (o1 ? zhm1 : 0u);
                         }
+                    }
+                    if (HP) {
+                        // the coordinate again in fp64: cell and position in the cell from it (the fp32 value above only
+                        // serves the guard-band logic, whose band is far wider than its error)
+#pragma unroll
+                        for (int rr = 0; rr < R; ++rr) {
+                            if (!((mask >> rr) & 1)) continue;
+                            const double t64 = fma(pd.Bs, one_minus_cos_poly_f64(fma(jd, pd.dphi, dcr64[rr])), pd.A);
+                            const int cell = min(__double2int_rd(t64), 0x3FFFFF);
+                            gt[rr] = (float)(t64 - (double)cell) - 0.5f;
+                            gc[rr] = kMagicBits + (unsigned)cell;
+                            cb[rr] = gc[rr];
+                        }
+                        jd += 1.0;
                     }
                     // cells below the last: plain lookup; beyond the zero cell: clamp onto it (weight 0);
                     // the last cell and the zero cell (t in [tmax - 1, tmax + 1)) take the branch
@@ -618,17 +643,17 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     }
 }
 
-template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR>
+template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR, bool HP = false>
 static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st) {
     const char *dbg = std::getenv("SC_DBG");
-    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0, L.tile_ctr};
+    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0, L.pairsd, L.tile_ctr};
     static bool attr_done[64] = {};
-    cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR>, attr_done);
+    cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = std::min(L.nsm, L.ntiles);
     if (grid <= 0) return cudaSuccess;
     if ((e = cudaMemsetAsync(L.tile_ctr, 0, sizeof(int), st)) != cudaSuccess) return e;      // the launch's tile counter
-    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 

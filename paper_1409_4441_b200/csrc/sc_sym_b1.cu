@@ -10,6 +10,20 @@ cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cu
     const bool z = P.zoned != 0;
 #define SC_GO(R, NC, TOT, TM, SOUTH, MIRROR) \
     return z ? launch_sym<1, R, NC, TOT, true, TM, SOUTH, MIRROR>(L, P, io, st) : launch_sym<1, R, NC, TOT, false, TM, SOUTH, MIRROR>(L, P, io, st)
+    if (P.hp) {                                         // fp64 table coordinate (steep tables), full-sphere instances only
+        if (!L.south || z || !L.pairsd) return cudaErrorInvalidValue;
+        if (L.mirror) {
+            if (L.threads != 192 || L.R != 4) return cudaErrorInvalidValue;
+            if (L.tot && L.tmem) return launch_sym<1, 4, 192, true, false, true, true, true, true>(L, P, io, st);
+            if (!L.tot && !L.tmem) return launch_sym<1, 4, 192, false, false, false, true, true, true>(L, P, io, st);
+            return cudaErrorInvalidValue;
+        }
+        if (!L.tot || L.tmem) return cudaErrorInvalidValue;      // large discs whose runs do not fit the 16-image tiles
+        if (L.threads == 256 && L.R == 4) return launch_sym<1, 4, 256, true, false, false, true, false, true>(L, P, io, st);
+        if (L.threads == 256 && L.R == 2) return launch_sym<1, 2, 256, true, false, false, true, false, true>(L, P, io, st);
+        if (L.threads == 128 && L.R == 2) return launch_sym<1, 2, 128, true, false, false, true, false, true>(L, P, io, st);
+        return cudaErrorInvalidValue;
+    }
     if (L.south && L.mirror) {                          // 16 images
         if (L.threads == 192 && L.R == 4 && L.tot && L.tmem) { SC_GO(4, 192, true, true, true, true); }
         if (L.threads == 192 && L.R == 4 && !L.tot && !L.tmem) { SC_GO(4, 192, false, false, true, true); }

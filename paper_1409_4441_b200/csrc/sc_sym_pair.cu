@@ -477,7 +477,7 @@ sym_pair_kernel(const Dev P, const FastDev F, const Maps io) {
 template <int NCW, int NPW, bool TOT, bool Z, bool SOUTH>
 static cudaError_t launch_pair(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st) {
     const char *dbg = std::getenv("SC_DBG");
-    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0, nullptr};
+    FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0, nullptr, nullptr};
     static bool attr_done[64] = {};
     cudaError_t e = ensure_max_smem(sym_pair_kernel<NCW, NPW, TOT, Z, SOUTH>, attr_done);
     if (e != cudaSuccess) return e;
