@@ -561,6 +561,8 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         // one map per launch: 16 images per pair geometry (mirror symmetry as well) -- half the table gathers and
         // geometry per pair; twice the staged bytes per base pixel, so 192 consumer threads x 4 base pixels
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR")) cands.insert(cands.begin(), Cand{192, 4, true});
+        // ... or 256 consumer threads x 3 base pixels: the same 768-pixel tiles with 8 consumer warps
+        if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && !std::getenv("SC_SYM_NOR3")) cands.insert(cands.begin(), Cand{256, 3, true});
         // ... and as lane pairs (sc_sym_pair.cu): 32 accumulators per lane, 12 (small discs) or 8 consumer warps
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && std::getenv("SC_SYM_PAIR"))
             cands.insert(cands.begin(), mean_nb <= 700.0 ? Cand{env_int("SC_PAIR_NC", 384), 4, true, true} : Cand{256, 4, true, true});

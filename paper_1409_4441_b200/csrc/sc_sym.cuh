@@ -81,7 +81,7 @@ static __device__ __noinline__ unsigned sym_exact_mask(const Dev &P, int r, int 
 // index of the 8-position block spreads such a stride over all 8 bank groups for every alignment, with no
 // padding (brute-force checked: 1 wavefront per quarter warp for stride 2 and 4; stride 1 needs nothing).
 template <int R> __host__ __device__ __forceinline__ int slot_of_pos(int i) {
-    return R == 1 ? i : (R == 2 ? i ^ ((i >> 3) & 1) : i ^ ((i >> 3) & 3));
+    return (R == 1 || R == 3) ? i : (R == 2 ? i ^ ((i >> 3) & 1) : i ^ ((i >> 3) & 3));     // stride 3 is coprime with the 8 bank groups
 }
 
 // Packed fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a; a scalar operand is broadcast by the hardware).
@@ -102,6 +102,9 @@ constexpr int kSymBuf = 2;        // stage buffers
 #ifndef SC_L192
 #define SC_L192 1
 #endif
+#ifndef SC_R3_PIPE
+#define SC_R3_PIPE 0
+#endif
 __host__ __device__ constexpr int sym_nprod(int NC) { return (NC == 192 && SC_L192 == 1) ? 64 : 128; }
 // SC_L192 == 0 (A/B layout): warps 0-5 = consumers, 6-7 = idle (they exit after the register hand-over of their
 // warpgroup: setmaxnreg works on whole warpgroups), 8-11 = producers.
@@ -116,7 +119,7 @@ __host__ __device__ constexpr int sym_tmem_cols(int NC, int per_thread) {
 
 // Per-position state of the pair loop: lookup coordinate - 1/2 and table cell bits of the R pixels (geometry stage),
 // table cells and map values (load stage)
-template <int R> struct SymGeo { float t[R < 2 ? 2 : R]; unsigned c[R < 2 ? 2 : R]; };
+template <int R> struct SymGeo { float t[2 * ((R + 1) / 2)]; unsigned c[2 * ((R + 1) / 2)]; };
 template <int R, int B, int NPL> struct SymLd { float2 el[R]; float4 mv[B][NPL]; };
 
 // Tile n of this CTA: rows of gridDim.x tiles, alternate rows reversed ("snake") so that the CTAs
@@ -140,7 +143,7 @@ template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRR
 __global__ void __launch_bounds__(sym_threads(NC), 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(!(HP && Z), "the fp64 coordinate is not combined with the two-zone table");
-    static_assert(R == 1 || R == 2 || R == 4, "R");
+    static_assert(R >= 1 && R <= 4, "R");
     constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
     constexpr int NPROD = sym_nprod(NC), PROD0 = sym_prod0(NC);
     constexpr int NPL = sym_planes(SOUTH, MIRROR);       // staged planes per position, 4 rotation images each
@@ -408,7 +411,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 const unsigned zhm1 = (unsigned)P.z_hm1;
                 float2 dc2[RP];
 #pragma unroll
-                for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[R > 1 ? 2 * h + 1 : 0]);
+                for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[2 * h + 1 < R ? 2 * h + 1 : 2 * h]);
                 float2 jf = f2((float)(-pe.hw));
                 const int pos0 = i0 - pe.hw, pend = i0 + pe.hw + R - 1;
                 // One window position for the pixels rr in MASK (compile time).  The window of the thread is the
@@ -529,14 +532,15 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 const bool peel = R > 1 && 2 * pe.hw >= R - 2;       // first and last R - 1 positions do not overlap
                 if (peel) {
                     body(pos++, std::integral_constant<int, 1>{});
-                    if (R == 4) { body(pos++, std::integral_constant<int, 3>{}); body(pos++, std::integral_constant<int, 7>{}); }
+                    if (R >= 3) body(pos++, std::integral_constant<int, 3>{});
+                    if (R == 4) body(pos++, std::integral_constant<int, 7>{});
                     plast = pend - (R - 1);
                 }
                 // Main positions (all R pixels), software-pipelined over two register sets: the loads of position
                 // i + 1 are issued before the FMAs of position i, the geometry of position i + 2 after them.  The
                 // number of positions is the same for all lanes (2 hw + R - 2 (R - 1) or 2 hw + R).
                 int left = plast - pos + 1;
-                constexpr bool PIPE = NC == 192;                     // only the 6-warp instance needs it (elsewhere: spills, slower)
+                constexpr bool PIPE = NC == 192 || (R == 3 && SC_R3_PIPE);                     // only the 6-warp instance needs it (elsewhere: spills, slower)
                 if (!PIPE) {
 #pragma unroll 2
                     for (; pos <= plast; ++pos) body(pos, ALL);
@@ -558,7 +562,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     }
                 }
                 if (peel) {
-                    if (R == 4) { body(pos++, std::integral_constant<int, 14 & kAll>{}); body(pos++, std::integral_constant<int, 12 & kAll>{}); }
+                    if (R == 4) body(pos++, std::integral_constant<int, 14 & kAll>{});
+                    if (R >= 3) body(pos++, std::integral_constant<int, (3 << (R >= 2 ? R - 2 : 0)) & kAll>{});
                     body(pos++, std::integral_constant<int, (1 << (R - 1))>{});
                 }
                 if (TOT && TM) {                                 // totals (tensor memory) += this ring's sums

@@ -25,6 +25,8 @@ cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cu
         return cudaErrorInvalidValue;
     }
     if (L.south && L.mirror) {                          // 16 images
+        if (L.threads == 256 && L.R == 3 && L.tot && L.tmem) { SC_GO(3, 256, true, true, true, true); }
+        if (L.threads == 256 && L.R == 3 && !L.tot && !L.tmem) { SC_GO(3, 256, false, false, true, true); }
         if (L.threads == 192 && L.R == 4 && L.tot && L.tmem) { SC_GO(4, 192, true, true, true, true); }
         if (L.threads == 192 && L.R == 4 && !L.tot && !L.tmem) { SC_GO(4, 192, false, false, true, true); }
         return cudaErrorInvalidValue;
