@@ -17,7 +17,7 @@ namespace sc {
 
 enum { MODE_CONV = 0, MODE_COUNT = 1 };
 
-template <int B, int MODE>
+template <int B, int MODE, bool HP>
 __global__ void __launch_bounds__(128)
 generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
                int *__restrict__ count_out, unsigned long long *__restrict__ sig_out, Audit au,
@@ -58,7 +58,7 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
             // nearest pixel of ring rq in azimuth and the (small) offset to it
             const double xq = (phip - P.phi0[rq - 1]) / dphiq;
             int kc = (int)rint(xq);
-            const double dc64 = (P.phi0[rq - 1] + (double)kc * dphiq) - phip;
+            const double dc64 = (P.phi0[rq - 1] + (double)kc * dphiq) - phip;   // (kept in fp64 only if HP)
             const float dc = (float)dc64;
             kc %= nq; if (kc < 0) kc += nq;
             int jlo, jcnt;
@@ -93,7 +93,7 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
                         int i = (int)tt;
                         float xk = tt;                                  // K = tab[i].x + xk tab[i].y
                         if (P.zoned) zoned_cell(P, tt, i, xk);
-                        else if (P.hp) {                                // fp64 coordinate -> cell + position in the cell
+                        else if (HP) {                                  // fp64 coordinate -> cell + position in the cell
                             const double t64 = fmin(fma(sp * sq * P.scale, one_minus_cos_f64(fma((double)j, dphiq, dc64)), A64 * P.scale), (double)P.tmax);
                             i = min((int)t64, P.ntab - 2);
                             xk = (float)(t64 - (double)i);
@@ -133,7 +133,7 @@ generic_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1,
 // Same arithmetic with one WARP per output pixel: 4 groups of 8 lanes take every 4th input ring, the 8
 // lanes of a group share its azimuthal window, and the partial sums are combined with warp shuffles.  Used for the few thousand pixels next to
 // the poles, where one thread per pixel leaves the GPU almost empty (latency bound).
-template <int B>
+template <int B, bool HP>
 __global__ void __launch_bounds__(128)
 generic_warp_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1) {
     const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -199,7 +199,7 @@ generic_warp_kernel(const Dev P, const Maps io, int a0, int a1, int b0, int b1) 
                 int i = (int)tt;
                 float xk = tt;                                  // K = tab[i].x + xk tab[i].y
                 if (P.zoned) zoned_cell(P, tt, i, xk);
-                else if (P.hp) {                                // fp64 coordinate -> cell + position in the cell
+                else if (HP) {                                  // fp64 coordinate -> cell + position in the cell
                     const double t64 = fmin(fma(sp * sq * P.scale, one_minus_cos_f64(fma((double)j, dphiq, dc64)), A64 * P.scale), (double)P.tmax);
                     i = min((int)t64, P.ntab - 2);
                     xk = (float)(t64 - (double)i);
@@ -229,11 +229,16 @@ cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int
     if (n <= 0) return cudaSuccess;
     const int threads = 128, blocks = (n + threads - 1) / threads;
     Audit au{};
+    if (P.hp) {                                              // fp64 table coordinate: one map per launch (sc_plan.cu)
+        if (B != 1) return cudaErrorInvalidValue;
+        generic_kernel<1, MODE_CONV, true><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0);
+        return cudaGetLastError();
+    }
     switch (B) {
-        case 1: generic_kernel<1, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
-        case 2: generic_kernel<2, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
-        case 3: generic_kernel<3, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
-        case 4: generic_kernel<4, MODE_CONV><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
+        case 1: generic_kernel<1, MODE_CONV, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
+        case 2: generic_kernel<2, MODE_CONV, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
+        case 3: generic_kernel<3, MODE_CONV, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
+        case 4: generic_kernel<4, MODE_CONV, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1, nullptr, nullptr, au, 0); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -244,11 +249,16 @@ cudaError_t launch_generic_conv_warp(const Dev &P, const Maps &io, int B, int a0
     const int n = (a1 - a0) + (b1 - b0);
     if (n <= 0) return cudaSuccess;
     const int threads = 128, blocks = (n + 3) / 4;
+    if (P.hp) {
+        if (B != 1) return cudaErrorInvalidValue;
+        generic_warp_kernel<1, true><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1);
+        return cudaGetLastError();
+    }
     switch (B) {
-        case 1: generic_warp_kernel<1><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
-        case 2: generic_warp_kernel<2><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
-        case 3: generic_warp_kernel<3><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
-        case 4: generic_warp_kernel<4><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 1: generic_warp_kernel<1, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 2: generic_warp_kernel<2, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 3: generic_warp_kernel<3, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 4: generic_warp_kernel<4, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -261,7 +271,7 @@ cudaError_t launch_generic_count(const Dev &P, int *count_dev, unsigned long lon
     Maps io{};
     Audit a{};
     if (au) a = *au;
-    generic_kernel<0, MODE_COUNT><<<blocks, threads, 0, st>>>(P, io, 0, n, 0, 0, count_dev, sig_dev, a, au ? 1 : 0);
+    generic_kernel<0, MODE_COUNT, false><<<blocks, threads, 0, st>>>(P, io, 0, n, 0, 0, count_dev, sig_dev, a, au ? 1 : 0);
     return cudaGetLastError();
 }
 
