@@ -244,7 +244,7 @@ cudaError_t fast_launch_cap(FastPlan *fp, const Dev &P, const Maps &io, int ring
         std::vector<Cand> cands;
         if (fp->mean_nb <= 700.0) cands = {{384, 4}, {256, 4}, {128, 2}};
         else cands = {{256, 4}, {128, 2}};
-        const int Lmax = (int)(((size_t)fp->smem_optin - 256 - fp->tab_bytes) / ((size_t)kSymBufH * 2 * 16)) & ~7;
+        const int Lmax = (int)(((size_t)fp->smem_optin - 512 - fp->tab_bytes) / ((size_t)kSymBufH * 2 * 16)) & ~7;
         std::vector<SymTile> tiles;
         FastCfg c;
         for (const Cand &cd : cands) {
@@ -253,7 +253,7 @@ cudaError_t fast_launch_cap(FastPlan *fp, const Dev &P, const Maps &io, int ring
                 tiles.clear();
                 const int Lneed = build_sym_tiles(*fp->geo, cd.R, W, W * C - shrink, Lmax, s_hi, s_lo, true, tiles, true);
                 const size_t smem = fp->tab_bytes + (size_t)kSymBufH * 2 * Lneed * 16;
-                if (smem + 256 > (size_t)fp->smem_optin) continue;
+                if (smem + 512 > (size_t)fp->smem_optin) continue;
                 c.threads = cd.threads; c.R = cd.R; c.run = W * C - shrink; c.mirror = true; c.Ltot = Lneed; c.smem = smem;
                 c.tot = cd.threads != 384; c.tmem = false; c.ntiles = (int)tiles.size();
                 c.ok = true;
@@ -581,7 +581,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int run = W * C - shrink;
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int npl = cd.mirror ? 4 : 2;                      // staged planes per position (float4 of rotation images each)
-            const size_t stat = cd.pair ? 3072 : 256;            // static shared memory of the kernel (barriers; step records)
+            const size_t stat = cd.pair ? 3072 : 512;            // static shared memory of the kernel (barriers; step records)
             const int Lmax = (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
             HostGeo &g = *fp->geo;
             g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;

@@ -154,6 +154,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 127) & ~(size_t)127));
     __shared__ unsigned long long full_bar[kSymBuf], empty_bar[kSymBuf];
     __shared__ int s_tile[4];                            // tiles taken by this CTA (ring): written by producer 0, -1 = no more
+    __shared__ int4 s_run[2][kMaxSub][2];                // producers: the runs of a step {kq0, km0, L, nq}, {start_n, start_s, soff, -}
     const int tid = threadIdx.x;
     const int N = P.nside;
     const int Ltot = F.Ltot;
@@ -181,6 +182,33 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
         if (NC == 256 || NC == 384 || (NC == 192 && SC_L192 == 0)) asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
         const int pt = tid - PROD0;
         const int m = pt & 3;                            // quadrant image staged by this thread
+        // the run of sub-tile s at a step: first staged input pixel (rotation 0) and its reflected image, length, ring starts
+        auto run_of = [&](const SymTile *tl, int step, int s, int par) {
+            int4 ra = make_int4(0, 0, 0, 4), rb = make_int4(0, 0, 0, 0);
+            if (s < __ldg(&tl->nsub) && step < __ldg(&tl->sub[s].ne)) {
+                const int r = __ldg(&tl->sub[s].r), k0 = __ldg(&tl->sub[s].k0), n = __ldg(&tl->sub[s].n);
+                const PairEnt *pe = F.pairs + (__ldg(&tl->sub[s].e0) + step);
+                const int2 pa = __ldg(reinterpret_cast<const int2 *>(&pe->rq));       // rq, hw
+                const int2 pb = __ldg(reinterpret_cast<const int2 *>(&pe->ipq));      // ipq, shq
+                const int2 ps = __ldg(reinterpret_cast<const int2 *>(&pe->start_n));  // start_n, start_s
+                const int hw = pa.y, ipq = pb.x, shq = pb.y;
+                const int ips = r < N ? r : N;
+                const int shs = (r >= N) ? ((r - N) & 1) : 0;
+                const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
+                const int nq = 4 * ipq;
+                const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
+                const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw;
+                const int L = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R - w0;
+                int k = w0 + nq;                          // in [0, 2 nq): w0 >= -hw - 1 > -nq
+                if (k >= nq) k -= nq;
+                // mirror image of position i: pixel ipq - 1 + shq - (w0 + i), walking backwards
+                int km = (ipq - 1 + shq - w0) % nq;
+                if (km < 0) km += nq;
+                ra = make_int4(k, km, L, nq);
+                rb = make_int4(ps.x, ps.y, __ldg(&tl->sub[s].soff), 0);
+            }
+            s_run[par][s][0] = ra; s_run[par][s][1] = rb;
+        };
         // Dynamic schedule: the tile list is sorted by decreasing work and a CTA takes the next tile when it is done with
         // its last one (one atomicAdd per tile by producer 0, handed to the other threads through s_tile).
         for (int n = 0;; ++n) {
@@ -193,41 +221,27 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 break;
             }
             const SymTile *tl = F.tiles + tile;
-            const int nsub = __ldg(&tl->nsub), nsteps = __ldg(&tl->nsteps);
+            const int nsteps = __ldg(&tl->nsteps);
+            if (pt < kMaxSub) run_of(tl, 0, pt, it & 1);    // (the tile's first step: its runs are not known earlier)
             for (int step = 0; step < nsteps; ++step, ++it) {
                 const int buf = it % kSymBuf;
-                // runs to stage for this step, worked out BEFORE waiting for the buffer so that the
-                // table reads (global memory) are off the critical path
+                asm volatile("bar.sync 1, %0;" ::"n"(NPROD) : "memory");        // this step's runs are in s_run[it & 1]
+                // The runs to stage for this step (one per sub-tile) were worked out by producer threads 0 .. kMaxSub - 1 during
+                // the PREVIOUS step (run_of below) and handed over through s_run: nobody walks the dependent loads
+                // tile -> ring pair in every thread, and they are off the critical path.
                 int kq0[kMaxSub], km0[kMaxSub], Ls[kMaxSub], nqs[kMaxSub], sn[kMaxSub], ss[kMaxSub];
                 unsigned d0[kMaxSub];
 #pragma unroll
                 for (int s = 0; s < kMaxSub; ++s) {
-                    Ls[s] = 0;
-                    if (s >= nsub) continue;
-                    const int ne = __ldg(&tl->sub[s].ne);
-                    if (step >= ne) continue;
-                    const int r = __ldg(&tl->sub[s].r), k0 = __ldg(&tl->sub[s].k0), n = __ldg(&tl->sub[s].n);
-                    const int soff = __ldg(&tl->sub[s].soff);
-                    const PairEnt *pe = F.pairs + (__ldg(&tl->sub[s].e0) + step);
-                    const int2 pa = __ldg(reinterpret_cast<const int2 *>(&pe->rq));       // rq, hw
-                    const int2 pb = __ldg(reinterpret_cast<const int2 *>(&pe->ipq));      // ipq, shq
-                    const int2 ps = __ldg(reinterpret_cast<const int2 *>(&pe->start_n));  // start_n, start_s
-                    const int hw = pa.y, ipq = pb.x, shq = pb.y;
-                    const int ips = r < N ? r : N;
-                    const int shs = (r >= N) ? ((r - N) & 1) : 0;
-                    const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
-                    const int nq = 4 * ipq;
-                    const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
-                    const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw;
-                    Ls[s] = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R - w0;
-                    int k = w0 + m * ipq + nq;           // in [0, 2 nq)
-                    if (k >= nq) k -= nq;
-                    kq0[s] = k; nqs[s] = nq; sn[s] = ps.x; ss[s] = ps.y;
-                    // mirror image of position i: pixel (ipq - 1 + shq - (w0 + i)) + m ipq, walking backwards
-                    int km = ipq - 1 + shq - w0 + m * ipq;   // in (-nq, 2 nq + ...): w0 >= -hw - 1 > -ipq
-                    km %= nq; if (km < 0) km += nq;
+                    const int4 ra = s_run[it & 1][s][0], rb = s_run[it & 1][s][1];
+                    Ls[s] = ra.z; nqs[s] = ra.w; sn[s] = rb.x; ss[s] = rb.y;
+                    int k = ra.x + m * (ra.w >> 2);           // rotation m of the first staged pixel
+                    if (k >= ra.w) k -= ra.w;
+                    kq0[s] = k;
+                    int km = ra.y + m * (ra.w >> 2);
+                    if (km >= ra.w) km -= ra.w;
                     km0[s] = km;
-                    d0[s] = stage_sh + (unsigned)((buf * B * NPL) * Ltot + soff) * 16u + 4u * m;
+                    d0[s] = stage_sh + (unsigned)((buf * B * NPL) * Ltot + rb.z) * 16u + 4u * m;
                 }
                 mbar_wait_sleep(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);   // every consumer warp released it
 #pragma unroll
@@ -275,6 +289,9 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     }
                 }
                 cp_async_mbar_arrive(&full_bar[buf]);   // arrives when this thread's copies have landed
+                // ... and the runs of the next step, while the copies are in flight (of this tile: the first step of the next
+                // tile is done at its start)
+                if (pt < kMaxSub && step + 1 < nsteps) run_of(tl, step + 1, pt, (it + 1) & 1);
             }
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
