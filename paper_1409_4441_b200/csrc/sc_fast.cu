@@ -568,7 +568,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             cands.insert(cands.begin(), mean_nb <= 700.0 ? Cand{env_int("SC_PAIR_NC", 384), 4, true, true} : Cand{256, 4, true, true});
         if (P.hp) {                                         // fp64 table coordinate: the 16-image instance only, one map per launch
             if (B > 1) continue;
-            cands = {Cand{192, 4, true}, Cand{256, 4, false}, Cand{256, 2, false}, Cand{128, 2, false}};
+            cands = {Cand{256, 3, true}, Cand{192, 4, true}, Cand{256, 4, false}, Cand{256, 2, false}, Cand{128, 2, false}};
         }
         const int fr = env_int("SC_SYM_R", 0), ft = env_int("SC_SYM_THREADS", 0);
         if (!P.hp && fr > 0 && ft > 0 && (fr == 1 || fr == 2 || (fr == 4 && B <= 2)) && (ft == 128 || ft == 256 || (ft == 384 && fr == 4 && B == 1)))

@@ -12,6 +12,11 @@ cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cu
     return z ? launch_sym<1, R, NC, TOT, true, TM, SOUTH, MIRROR>(L, P, io, st) : launch_sym<1, R, NC, TOT, false, TM, SOUTH, MIRROR>(L, P, io, st)
     if (P.hp) {                                         // fp64 table coordinate (steep tables), full-sphere instances only
         if (!L.south || z || !L.pairsd) return cudaErrorInvalidValue;
+        if (L.mirror && L.threads == 256 && L.R == 3) {
+            if (L.tot && L.tmem) return launch_sym<1, 3, 256, true, false, true, true, true, true>(L, P, io, st);
+            if (!L.tot && !L.tmem) return launch_sym<1, 3, 256, false, false, false, true, true, true>(L, P, io, st);
+            return cudaErrorInvalidValue;
+        }
         if (L.mirror) {
             if (L.threads != 192 || L.R != 4) return cudaErrorInvalidValue;
             if (L.tot && L.tmem) return launch_sym<1, 4, 192, true, false, true, true, true, true>(L, P, io, st);
