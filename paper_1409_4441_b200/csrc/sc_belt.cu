@@ -118,6 +118,9 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
     const int tid = threadIdx.x, lane = tid & 31;
     const int N = P.nside, N4 = 4 * N;
     const int NBUF = F.nbuf, NTB = F.ntb;
+    // a kernel launched behind this one with programmatic stream serialization (the sym kernel: disjoint outputs, no
+    // wait on this grid) may take the SMs as this kernel's CTAs leave them
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     float *stage = reinterpret_cast<float *>(smem_raw);                           // [NBUF][8][LP]
     const TapLayout TL(F.pw_max, F.ne_max);
     unsigned char *tapbase = smem_raw + (size_t)NBUF * 8 * LP * 4;                // [NTB] tap buffers

@@ -60,6 +60,8 @@ struct SymLaunch {
     bool pair;                  // lane-pair instance (sc_sym_pair.cu): two lanes share a group of R base pixels
     int *tile_ctr;              // plan-owned device counter for the dynamic tile schedule
     const PairEntD *pairsd;     // fp64 ring pairs of a Dev::hp plan
+    bool overlap;               // launch with programmatic stream serialization: the CTAs may start while the previous kernel of
+                                // the stream (the belt kernel: disjoint outputs) drains; the tile counter was zeroed before that kernel
 };
 cudaError_t dispatch_sym_pair(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
 cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);

@@ -244,24 +244,37 @@ cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int
     return cudaGetLastError();
 }
 
+// overlap: launched with programmatic stream serialization -- the blocks may start while the previous kernel of the stream
+// (a fast kernel: disjoint outputs, same inputs) drains
+template <int B, bool HP>
+static cudaError_t launch_warp(const Dev &P, const Maps &io, int a0, int a1, int b0, int b1, int blocks, int threads, cudaStream_t st,
+                               bool overlap) {
+    if (!overlap) {
+        generic_warp_kernel<B, HP><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1);
+        return cudaGetLastError();
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(blocks); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at{};
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, generic_warp_kernel<B, HP>, P, io, a0, a1, b0, b1);
+}
+
 cudaError_t launch_generic_conv_warp(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1,
-                                     cudaStream_t st) {
+                                     cudaStream_t st, bool overlap) {
     const int n = (a1 - a0) + (b1 - b0);
     if (n <= 0) return cudaSuccess;
     const int threads = 128, blocks = (n + 3) / 4;
-    if (P.hp) {
-        if (B != 1) return cudaErrorInvalidValue;
-        generic_warp_kernel<1, true><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1);
-        return cudaGetLastError();
-    }
+    if (P.hp) return B == 1 ? launch_warp<1, true>(P, io, a0, a1, b0, b1, blocks, threads, st, overlap) : cudaErrorInvalidValue;
     switch (B) {
-        case 1: generic_warp_kernel<1, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
-        case 2: generic_warp_kernel<2, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
-        case 3: generic_warp_kernel<3, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
-        case 4: generic_warp_kernel<4, false><<<blocks, threads, 0, st>>>(P, io, a0, a1, b0, b1); break;
+        case 1: return launch_warp<1, false>(P, io, a0, a1, b0, b1, blocks, threads, st, overlap);
+        case 2: return launch_warp<2, false>(P, io, a0, a1, b0, b1, blocks, threads, st, overlap);
+        case 3: return launch_warp<3, false>(P, io, a0, a1, b0, b1, blocks, threads, st, overlap);
+        case 4: return launch_warp<4, false>(P, io, a0, a1, b0, b1, blocks, threads, st, overlap);
         default: return cudaErrorInvalidValue;
     }
-    return cudaGetLastError();
 }
 
 cudaError_t launch_generic_count(const Dev &P, int *count_dev, unsigned long long *sig_dev,

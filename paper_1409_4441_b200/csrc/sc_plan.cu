@@ -14,7 +14,8 @@
 
 namespace sc {
 cudaError_t launch_generic_conv(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1, cudaStream_t st);
-cudaError_t launch_generic_conv_warp(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1, cudaStream_t st);
+cudaError_t launch_generic_conv_warp(const Dev &P, const Maps &io, int B, int a0, int a1, int b0, int b1, cudaStream_t st,
+                                     bool overlap = false);
 cudaError_t launch_generic_count(const Dev &P, int *count_dev, unsigned long long *sig_dev, const Audit *au, cudaStream_t st);
 struct FastPlan;
 FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std::vector<double> &s,
@@ -446,9 +447,13 @@ static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps,
             if (ev) { SC_CUDA(cudaEventRecord(ev[1], st)); SC_CUDA(cudaEventRecord(ev[2], st)); SC_CUDA(cudaEventRecord(ev[3], st)); }
         } else {
             // rings next to the poles: generic kernel; everything else: fast kernels
+            // (the three kernels write disjoint pixels: unless every kernel is being timed, the warp-per-pixel kernel goes
+            // last and may start while the sym kernel drains)
             const int pr = plan->polar_rings;
-            if (pr > 0) {
-                const int np = 2 * pr * (pr + 1);          // pixels in rings 1..pr
+            const int np = 2 * pr * (pr + 1);              // pixels in rings 1..pr
+            const bool polar_last = !ev && !std::getenv("SC_NO_OVERLAP") &&
+                                    0.5 * (double)D.npix * ((double)D.tmax / D.scale) <= 8000.0;      // discs below ~8000 pixels only: at config 6 (61000) the 36 ms polar kernel last costs +6 %
+            if (pr > 0 && !polar_last) {
                 SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, st));
                 ++launches;
             }
@@ -456,6 +461,10 @@ static sc_status convolve_impl(const sc_plan *plan, const float *const *in_maps,
             int nl = 0;
             SC_CUDA(sc::fast_convolve(plan->fast, D, io, nb, st, &nl, ev ? ev + 2 : nullptr));
             launches += nl;
+            if (pr > 0 && polar_last) {
+                SC_CUDA(sc::launch_generic_conv_warp(D, io, nb, 0, np, D.npix - np, D.npix, st, true));
+                ++launches;
+            }
         }
         if (plan->nested) {                                                // RING results -> NESTED outputs
             for (int b = 0; b < nb; ++b) SC_CUDA(sc::reorder_f32(D.nside, 1, plan->nest_out + npix * b, out_maps[b0 + b], st));

@@ -159,6 +159,9 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     const int N = P.nside;
     const int Ltot = F.Ltot;
 
+    // a kernel launched behind this one with programmatic stream serialization (the warp-per-pixel kernel: disjoint outputs,
+    // no wait on this grid) may take the SMs as this kernel's CTAs leave them
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     for (int i = tid; i < F.ntab_s; i += blockDim.x) tab[i] = P.tabh[i];
     if (tid == 0) {
         for (int i = 0; i < kSymBuf; ++i) { mbar_init(&full_bar[i], NPROD); mbar_init(&empty_bar[i], NC / 32); }
@@ -674,6 +677,15 @@ static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, 
     if (e != cudaSuccess) return e;
     const int grid = std::min(L.nsm, L.ntiles);
     if (grid <= 0) return cudaSuccess;
+    if (L.overlap) {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(sym_threads(NC)); cfg.dynamicSmemBytes = L.smem; cfg.stream = st;
+        cudaLaunchAttribute at{};
+        at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at.val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = &at; cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP>, P, F, io);
+    }
     if ((e = cudaMemsetAsync(L.tile_ctr, 0, sizeof(int), st)) != cudaSuccess) return e;      // the launch's tile counter
     sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
     return cudaGetLastError();
