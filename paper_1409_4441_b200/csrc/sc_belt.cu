@@ -98,22 +98,48 @@ __device__ __forceinline__ void bar_named(int id, int n) { asm volatile("bar.syn
 // Window of input ring `pe` for the tile starting at base pixel k0 of a ring with shift flag sh:
 // first staged position is w0a (multiple of 4), the window proper starts a0 positions later and the
 // consumers walk ng chunks of 4 positions.
+// PX: consecutive pixels owned by a consumer thread (4 or 8): its window is 2 hw + PX positions.
+template <int PX>
 __device__ __forceinline__ void belt_window(const PairEnt &pe, int sh, int k0, int &delta, int &w0a, int &a0, int &ng) {
     delta = (1 - sh + pe.shq) >> 1;
     const int first_pos = k0 + delta - pe.hw;
     w0a = first_pos & ~3;
     a0 = first_pos - w0a;
-    ng = (2 * pe.hw + 4 + a0 + 3) >> 2;
+    ng = (2 * pe.hw + PX + a0 + 3) >> 2;
+}
+
+// Edge masks of the 8-pixel consumers: bit 4 p + i = the FFMA2 of pixel pair p (pixels 2p, 2p + 1) at chunk position i
+// has a tap that can be non-zero.  Front chunk c (0, 1) with alignment a0: position 4c + i >= a0 + 2p.  Back chunk
+// (cl = 1: the last, 0: the one before) with remq = the last chunk's last position that pixel pair 3 uses:
+// i <= remq + 4 (1 - cl) - 2 (3 - p).
+__host__ __device__ constexpr unsigned belt_front_mask(int c, int a0) {
+    unsigned m = 0;
+    for (int p = 0; p < 4; ++p)
+        for (int i = 0; i < 4; ++i)
+            if (4 * c + i >= a0 + 2 * p) m |= 1u << (4 * p + i);
+    return m;
+}
+__host__ __device__ constexpr unsigned belt_back_mask(int cl, int remq) {
+    unsigned m = 0;
+    for (int p = 0; p < 4; ++p)
+        for (int i = 0; i < 4; ++i)
+            if (i <= remq + 4 * (1 - cl) - 2 * (3 - p)) m |= 1u << (4 * p + i);
+    return m;
 }
 
 
 // SLACK: floats per staged plane beyond the tile (window + alignment); TOT: second accumulator set
 // (flushed every >= 48 taps; needed for discs of thousands of pixels, costs 32 registers).
 // TM: the second accumulator set lives in tensor memory (512-consumer variant for large discs).
-template <int NC, int SLACK, bool TOT, bool TM>
+// W8: a consumer thread owns 8 consecutive pixels x 4 images (the images of one hemisphere) instead of 4 x 8: a staged
+// value then feeds 8 pixels, i.e. 4 map LDS.128 + 5 tap LDS.128 per 64 FFMA2 instead of 8 + 3.  The lanes' windows are
+// then 32 bytes apart, so lanes 4-7 of every 8 read the image planes in the order (1, 0, 3, 2) and the plane stride is
+// 4 floats off a multiple of 32: the 8 lanes of a quarter warp then cover all 32 banks.
+template <int NC, int SLACK, bool TOT, bool TM, bool W8>
 __global__ void __launch_bounds__(NC + kBeltProd, 1)
 belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
-    constexpr int T = 4 * NC, LP = T + SLACK;
+    constexpr int PX = W8 ? 8 : 4;
+    constexpr int T = 4 * NC, LP = T + SLACK + (W8 ? 4 : 0);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31;
     const int N = P.nside, N4 = 4 * N;
@@ -162,8 +188,8 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                         const PairEnt pe = pe_next;
                         if (e + 1 < ne) pe_next = F.pairs[e0 + e + 1];      // prefetched while waiting below
                         int delta, w0a, a0, ng;
-                        belt_window(pe, sh, k0, delta, w0a, a0, ng);
-                        const int len = T - 4 + 4 * ng;                       // floats per plane
+                        belt_window<PX>(pe, sh, k0, delta, w0a, a0, ng);
+                        const int len = T - PX + 4 * ng;                      // floats per plane
                         unsigned long long *bar = &full_bar[buf];
                         mbar_wait_sleep(&empty_bar[buf], par ^ 1u);           // every consumer warp released it
                         if (lane == 0) mbar_expect_tx(bar, (unsigned)(8 * len * 4));
@@ -209,7 +235,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     const PairEnt pe = F.pairs[e0 + e];
                     const int wo = F.woff[e0 + e];
                     int delta, w0a, a0, ng;
-                    belt_window(pe, sh, k0, delta, w0a, a0, ng);
+                    belt_window<PX>(pe, sh, k0, delta, w0a, a0, ng);
                     if (pt == 0) desc[e - ge0] = make_int4(ng, wo * 8, 2 * pe.hw + 1, a0);
                     // nearest pixel of ring rq in azimuth: kc = k + delta, at angle dcc from p.  In the belt
                     // Y = N (2k + 1 - sh + shq), so delta = (1 - sh + shq) >> 1 and the remainder is N or 0.
@@ -218,10 +244,10 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     PairEntD pd{};
                     if (P.hp) pd = F.pairsd[e0 + e];
                     const double dcc64 = (double)(N - ((Yk & 1) ? N : 0)) * pd.cdc;
-                    // S[i] = (w[x], w[x-1]), x = i - 2 - a0: chunk g of 4 staged positions uses S[4g .. 4g+5]
-                    const int nS = 4 * ng + 2;
+                    // S[i] = (w[x], w[x-1]), x = i - (PX - 2) - a0: chunk g of 4 staged positions uses S[4g .. 4g + PX + 1]
+                    const int nS = 4 * ng + PX - 2;
                     for (int i = pt; i < nS; i += kTapThreads) {
-                        const int x = i - 2 - a0;
+                        const int x = i - (PX - 2) - a0;
                         float w2[2];
 #pragma unroll
                         for (int q = 0; q < 2; ++q) {
@@ -253,6 +279,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
     if (NC == 512) asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
     int buf = 0; unsigned par = 0;
     int tb = 0; unsigned tpar = 0;
+    const int half = W8 ? tid / (NC / 2) : 0, u8 = W8 ? tid % (NC / 2) : 0, sk = W8 ? (lane >> 2) & 1 : 0;   // (W8) hemisphere, 8-pixel group, plane order
     const unsigned taddr = TM ? s_tmem + ((((unsigned)(tid >> 5) & 3u) * 32u) << 16) + ((unsigned)tid >> 7) * 32u : 0u;
     for (int row = 0; row < nrows; ++row) {
         const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
@@ -282,8 +309,71 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
             for (int e = ge0; e < ge1; ++e) {
                 const int4 d = desc[e - ge0];                             // (chunks, tap offset in bytes, taps)
                 const float4 *S4 = reinterpret_cast<const float4 *>(tbuf + d.y);   // S4[2 g + i] = S[4 g + 2 i .. + 1]
-                const float *pl = stage + (size_t)buf * 8 * LP + 4 * tid;
                 mbar_wait(&full_bar[buf], par);
+                if constexpr (W8) {
+                // chunk g4 = 4 staged positions x 4 images: 5 LDS.128 of tap pairs (broadcast) + 4 LDS.128 of map values,
+                // then 64 FFMA2.  Slot s of this thread is image 4 half + (s ^ sk); pixel pair p of slot s lives in
+                // acc01[s], acc23[s], acc01[4 + s], acc23[4 + s] for p = 0 .. 3.
+                const float *pl0 = stage + (size_t)buf * 8 * LP + (size_t)(4 * half) * LP + 8 * u8;
+                const float *pA = pl0 + sk * LP, *pB = pl0 - sk * LP;     // even / odd slots
+                float4 tp[5], mv[4];
+                auto load8 = [&](int g4) {
+#pragma unroll
+                    for (int i = 0; i < 5; ++i) tp[i] = S4[2 * g4 + i];
+                    mv[0] = *reinterpret_cast<const float4 *>(pA + 4 * g4);
+                    mv[1] = *reinterpret_cast<const float4 *>(pB + LP + 4 * g4);
+                    mv[2] = *reinterpret_cast<const float4 *>(pA + 2 * LP + 4 * g4);
+                    mv[3] = *reinterpret_cast<const float4 *>(pB + 3 * LP + 4 * g4);
+                };
+                auto fma8 = [&](auto MK) {
+                    constexpr unsigned mk = decltype(MK)::value;
+                    // pairs (w[x], w[x-1]) of the 10 tap positions this chunk touches: pixel pair p at position i uses pwr[6 - 2p + i]
+                    const float2 pwr[10] = {make_float2(tp[0].x, tp[0].y), make_float2(tp[0].z, tp[0].w), make_float2(tp[1].x, tp[1].y),
+                                            make_float2(tp[1].z, tp[1].w), make_float2(tp[2].x, tp[2].y), make_float2(tp[2].z, tp[2].w),
+                                            make_float2(tp[3].x, tp[3].y), make_float2(tp[3].z, tp[3].w), make_float2(tp[4].x, tp[4].y),
+                                            make_float2(tp[4].z, tp[4].w)};
+#pragma unroll
+                    for (int sl = 0; sl < 4; ++sl) {
+                        const float mm[4] = {mv[sl].x, mv[sl].y, mv[sl].z, mv[sl].w};
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const float2 m2 = make_float2(mm[i], mm[i]);
+                            if ((mk >> i) & 1) acc01[sl] = __ffma2_rn(pwr[6 + i], m2, acc01[sl]);
+                            if ((mk >> (4 + i)) & 1) acc23[sl] = __ffma2_rn(pwr[4 + i], m2, acc23[sl]);
+                            if ((mk >> (8 + i)) & 1) acc01[4 + sl] = __ffma2_rn(pwr[2 + i], m2, acc01[4 + sl]);
+                            if ((mk >> (12 + i)) & 1) acc23[4 + sl] = __ffma2_rn(pwr[i], m2, acc23[4 + sl]);
+                        }
+                    }
+                };
+#define SC_MK(m) std::integral_constant<unsigned, (m)>{}
+                const int ng = d.x, a0 = d.w;
+                int g4 = 0, gend = ng;
+                if (ng >= 4) {                                            // (else: every chunk with the full body, the taps are 0 there)
+                    switch (a0) {
+                        case 0: load8(0); fma8(SC_MK(belt_front_mask(0, 0))); load8(1); fma8(SC_MK(belt_front_mask(1, 0))); break;
+                        case 1: load8(0); fma8(SC_MK(belt_front_mask(0, 1))); load8(1); fma8(SC_MK(belt_front_mask(1, 1))); break;
+                        case 2: load8(0); fma8(SC_MK(belt_front_mask(0, 2))); load8(1); fma8(SC_MK(belt_front_mask(1, 2))); break;
+                        default: load8(0); fma8(SC_MK(belt_front_mask(0, 3))); load8(1); fma8(SC_MK(belt_front_mask(1, 3))); break;
+                    }
+                    g4 = 2; gend = ng - 2;
+                }
+#pragma unroll 1
+                for (; g4 < gend; ++g4) {
+                    load8(g4);
+                    fma8(SC_MK(0xFFFFu));
+                }
+                if (ng >= 4) {
+                    const int remq = a0 + d.z + 6 - 4 * (ng - 1);         // 0 .. 3
+                    switch (remq) {
+                        case 0: load8(ng - 2); fma8(SC_MK(belt_back_mask(0, 0))); load8(ng - 1); fma8(SC_MK(belt_back_mask(1, 0))); break;
+                        case 1: load8(ng - 2); fma8(SC_MK(belt_back_mask(0, 1))); load8(ng - 1); fma8(SC_MK(belt_back_mask(1, 1))); break;
+                        case 2: load8(ng - 2); fma8(SC_MK(belt_back_mask(0, 2))); load8(ng - 1); fma8(SC_MK(belt_back_mask(1, 2))); break;
+                        default: load8(ng - 2); fma8(SC_MK(belt_back_mask(0, 3))); load8(ng - 1); fma8(SC_MK(belt_back_mask(1, 3))); break;
+                    }
+                }
+#undef SC_MK
+                } else {
+                const float *pl = stage + (size_t)buf * 8 * LP + 4 * tid;
                 // chunk g4 = 4 staged positions x 8 images: 3 LDS.128 of tap pairs (broadcast) + 8 LDS.128 of map
                 // values, then 64 FFMA2.  The loads of chunk g4 + 1 are issued before the FMAs of chunk g4.
                 float4 tp[2][3], mv[2][8];
@@ -356,6 +446,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                     }
                 }
 #undef SC_MASKS
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty_bar[buf]);            // this warp is done with the buffer
                 if (++buf == NBUF) { buf = 0; par ^= 1u; }
@@ -400,6 +491,26 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 for (int g = 0; g < 8; ++g) { tt[0][g] = s01[g].x; tt[1][g] = s01[g].y; tt[2][g] = s23[g].x; tt[3][g] = s23[g].y; }
                 auto apply = [&](const PairEnt &pe, int j, float Ku) {
                     const int delta = (1 - sh + pe.shq) >> 1;
+                    if constexpr (W8) {
+                        // pixel rr8 of this thread, slot sl: tt[rr8 & 3][4 (rr8 >> 2) + sl], image 4 half + (sl ^ sk)
+#pragma unroll
+                        for (int rr8 = 0; rr8 < 8; ++rr8) {
+                            const int k = k0 + 8 * u8 + rr8;
+                            const int kq = k + delta + j;
+                            const unsigned mask = belt_exact_mask(P, r, k, pe.rq, kq);
+                            int kqw = kq % N4; if (kqw < 0) kqw += N4;
+#pragma unroll
+                            for (int sl = 0; sl < 4; ++sl) {
+                                const int g = 4 * half + (sl ^ sk);
+                                if (mask & (1u << g)) {
+                                    int kk = kqw + (g & 3) * N; if (kk >= N4) kk -= N4;
+                                    tt[rr8 & 3][4 * (rr8 >> 2) + sl] =
+                                        fmaf(Ku, __ldg(in + (half ? pe.start_s : pe.start_n) + kk), tt[rr8 & 3][4 * (rr8 >> 2) + sl]);
+                                }
+                            }
+                        }
+                        return;
+                    }
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr) {
                         const int k = k0 + 4 * tid + rr;
@@ -460,6 +571,20 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
             const bool south = (r != 2 * N);
             const int k = k0 + 4 * tid;
             float *__restrict__ out = io.out[b];
+            if constexpr (W8) {                                   // 8 consecutive pixels per image -> two 16-byte stores
+                if (!half || south) {
+#pragma unroll
+                    for (int sl = 0; sl < 4; ++sl) {
+                        const int g = sl ^ sk;
+                        float *o = out + (half ? start_s : start_n) + k0 + 8 * u8 + g * N;
+                        *reinterpret_cast<float4 *>(o) = make_float4(tot01[sl].x * P.omega, tot01[sl].y * P.omega,
+                                                                     tot23[sl].x * P.omega, tot23[sl].y * P.omega);
+                        *reinterpret_cast<float4 *>(o + 4) = make_float4(tot01[4 + sl].x * P.omega, tot01[4 + sl].y * P.omega,
+                                                                         tot23[4 + sl].x * P.omega, tot23[4 + sl].y * P.omega);
+                    }
+                }
+                continue;
+            }
 #pragma unroll
             for (int g = 0; g < 8; ++g) {
                 if (g >= 4 && !south) break;
@@ -476,30 +601,35 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
 }
 
 // host ------------------------------------------------------------------------------------------
-size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_max) {
-    return (size_t)nbuf * 8 * (4 * NC + slack) * 4 + (size_t)ntb * TapLayout(pw_max, ne_max).bytes;
+size_t belt_smem_bytes(int NC, int slack, int px, int nbuf, int ntb, int pw_max, int ne_max) {
+    return (size_t)nbuf * 8 * (4 * NC + slack + (px == 8 ? 4 : 0)) * 4 + (size_t)ntb * TapLayout(pw_max, ne_max).bytes;
 }
 
-template <int NC, int SLACK, bool TOT, bool TM>
+template <int NC, int SLACK, bool TOT, bool TM, bool W8>
 static cudaError_t launch_belt_nc(const Dev &P, const BeltDev &F, const Maps &io, int B, size_t smem, int nsm, cudaStream_t st) {
     static bool attr_done[64] = {};
-    cudaError_t e = ensure_max_smem(belt_kernel<NC, SLACK, TOT, TM>, attr_done);
+    cudaError_t e = ensure_max_smem(belt_kernel<NC, SLACK, TOT, TM, W8>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = F.ntiles < nsm ? F.ntiles : nsm;
-    belt_kernel<NC, SLACK, TOT, TM><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
+    belt_kernel<NC, SLACK, TOT, TM, W8><<<grid, NC + kBeltProd, smem, st>>>(P, F, io, B);
     return cudaGetLastError();
 }
 
 // variants: (512 consumer threads, slack 64, single accumulator set) for small discs on Nside % 2048 == 0;
 // (256 | 128, slack 256 or 512, two accumulator sets) otherwise
-cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, size_t smem, int nsm,
-                        cudaStream_t st) {
-    if (threads == 512 && slack == 64) return launch_belt_nc<512, 64, false, false>(P, F, io, B, smem, nsm, st);
-    if (threads == 512 && slack == 256) return launch_belt_nc<512, 256, true, true>(P, F, io, B, smem, nsm, st);
-    if (threads == 512 && slack == 512) return launch_belt_nc<512, 512, true, true>(P, F, io, B, smem, nsm, st);
-    if (threads == 256 && slack == 256) return launch_belt_nc<256, 256, true, false>(P, F, io, B, smem, nsm, st);
-    if (threads == 256 && slack == 512) return launch_belt_nc<256, 512, true, false>(P, F, io, B, smem, nsm, st);
-    if (threads == 128 && slack == 256) return launch_belt_nc<128, 256, true, false>(P, F, io, B, smem, nsm, st);
+cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, int px, size_t smem,
+                        int nsm, cudaStream_t st) {
+#define SC_BELT(nc, sl, tot, tm)                                                                                          \
+    if (threads == nc && slack == sl)                                                                                     \
+        return px == 8 ? launch_belt_nc<nc, sl, tot, tm, true>(P, F, io, B, smem, nsm, st)                                \
+                       : launch_belt_nc<nc, sl, tot, tm, false>(P, F, io, B, smem, nsm, st);
+    SC_BELT(512, 64, false, false)
+    SC_BELT(512, 256, true, true)
+    SC_BELT(512, 512, true, true)
+    SC_BELT(256, 256, true, false)
+    SC_BELT(256, 512, true, false)
+    SC_BELT(128, 256, true, false)
+#undef SC_BELT
     return cudaErrorInvalidValue;
 }
 

@@ -20,8 +20,8 @@ constexpr int kSymBufH = 2;        // stage buffers of the sym kernel (kSymBuf i
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-size_t belt_smem_bytes(int NC, int slack, int nbuf, int ntb, int pw_max, int ne_max);
-cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, size_t smem, int nsm,
+size_t belt_smem_bytes(int NC, int slack, int px, int nbuf, int ntb, int pw_max, int ne_max);
+cudaError_t launch_belt(const Dev &P, const BeltDev &F, const Maps &io, int B, int threads, int slack, int px, size_t smem, int nsm,
                         cudaStream_t st);
 
 // Host geometry kept for building tile lists after plan creation (latitude bands)
@@ -143,7 +143,7 @@ struct FastPlan {
     int4 *belt_tiles = nullptr;
     std::vector<int> bch_off, bch_lo, bch_hi;   // belt latitude chunks (tile offsets, base rings), equator first
     std::shared_ptr<HostGeo> geo;
-    int belt_tiles_per_ring = 0, belt_slack = 0;
+    int belt_tiles_per_ring = 0, belt_slack = 0, belt_px = 4;   // belt_px: pixels per consumer thread (4 x 8 images or 8 x 4)
     int *grp_off = nullptr, *grp_e = nullptr;
     int *tile_ctr = nullptr;      // device counter of the sym kernel's dynamic tile schedule
     PairEntD *pairsd = nullptr;   // fp64 ring pairs (Dev::hp plans)
@@ -182,7 +182,7 @@ cudaError_t fast_launch(FastPlan *fp, const Dev &P, const Maps &io, int B, int w
             F.tiles += fp->bch_off[chunk]; F.ntiles = fp->bch_off[chunk + 1] - fp->bch_off[chunk];
         }
         if (F.ntiles > 0) {
-            e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_slack, fp->belt_smem, fp->nsm, st);
+            e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_slack, fp->belt_px, fp->belt_smem, fp->nsm, st);
             if (e == cudaSuccess) ++*launches;
         }
     }
@@ -220,7 +220,7 @@ cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, 
         BeltDev F = fp->belt;                               // tile list: ring 2N first, belt_tiles_per_ring tiles per ring
         F.tiles += (2 * N - b_hi) * fp->belt_tiles_per_ring;
         F.ntiles = (b_hi - b_lo + 1) * fp->belt_tiles_per_ring;
-        e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_slack, fp->belt_smem, fp->nsm, st);
+        e = launch_belt(P, F, io, B, fp->belt_threads, fp->belt_slack, fp->belt_px, fp->belt_smem, fp->nsm, st);
         if (e == cudaSuccess) ++*launches;
     }
     return e;
@@ -436,6 +436,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         if (N % 1024 == 0) { bvars.push_back({256, 256}); bvars.push_back({256, 512}); }
         else if (N % 512 == 0) bvars.push_back({128, 256});
     }
+    const int bpx = std::getenv("SC_BELT_PX4") ? 4 : 8;                   // pixels per consumer thread
     for (const BeltVar &bv : bvars) {
         if (no_belt || fp->belt_ok) break;
         const int bNC = bv.nc;
@@ -457,9 +458,9 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             int off = 0, cnt = 0;
             grp_e.push_back(0);
             for (size_t i = 0; i < per_ring[r].size(); ++i) {
-                const int ng_max = (2 * per_ring[r][i].hw + 4 + 3 + 3) >> 2;   // chunks of 4 staged positions
-                const int len = (4 * ng_max + 2 + 1) & ~1;                     // tap pairs, even count
-                if (all && (4 * ng_max > bv.slack + 4 || len > kTapCap)) fits = false;   // plane = T - 4 + 4 ng floats
+                const int ng_max = (2 * per_ring[r][i].hw + bpx + 3 + 3) >> 2; // chunks of 4 staged positions
+                const int len = (4 * ng_max + bpx - 2 + 1) & ~1;               // tap pairs, even count
+                if (all && (4 * ng_max > bv.slack + bpx || len > kTapCap)) fits = false;   // plane = T - px + 4 ng floats
                 if (cnt > 0 && (off + len > kTapCap || cnt >= kGroupRings)) {  // next group
                     grp_e.push_back((int)i); off = 0; cnt = 0;
                 }
@@ -479,7 +480,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         if (fits && !btiles.empty()) {
             const int combos[6][2] = {{2, 4}, {2, 3}, {1, 4}, {2, 2}, {1, 3}, {1, 2}};       // (tap buffers, stage buffers)
             for (const auto &cb : combos) {
-                bsmem = belt_smem_bytes(bNC, bv.slack, cb[1], cb[0], pw_max, ne_max);
+                bsmem = belt_smem_bytes(bNC, bv.slack, bpx, cb[1], cb[0], pw_max, ne_max);
                 if (bsmem + 2048 <= (size_t)smem_optin) { ntb = cb[0]; nbuf = cb[1]; break; }
             }
         }
@@ -493,7 +494,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((e = cudaMalloc((void **)&fp->grp_e, grp_e.size() * sizeof(int))) != cudaSuccess) return fail(e);
             if ((e = cudaMemcpy(fp->grp_e, grp_e.data(), grp_e.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) return fail(e);
             fp->belt = BeltDev{fp->pairs, fp->pair_off, fp->woff, fp->belt_tiles, fp->grp_off, fp->grp_e, (int)btiles.size(), pw_max, ne_max, nbuf, ntb, nullptr};
-            fp->belt_slack = bv.slack;
+            fp->belt_slack = bv.slack; fp->belt_px = bpx;
             fp->belt_threads = bNC; fp->belt_smem = bsmem; fp->belt_ok = true; fp->belt_tiles_per_ring = N / T;
             // latitude chunks: the tile list runs from ring 2N down to the first belt ring, N / T tiles per ring
             {
