@@ -215,7 +215,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 const int tile = row * G + ((row & 1) ? G - 1 - bid : bid);
                 if (tile >= F.ntiles) continue;
                 const int4 tl = F.tiles[tile];
-                const int r = tl.x, k0 = tl.y, ne = tl.w;
+                const int r = tl.x, k0 = tl.y;
                 const int sh = (r - N) & 1;
                 const int e0 = F.pair_off[tl.z];
                 const int g0 = F.grp_off[tl.z], ngrp = F.grp_off[tl.z + 1] - g0 - 1;
@@ -313,7 +313,10 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 if constexpr (W8) {
                 // chunk g4 = 4 staged positions x 4 images: 5 LDS.128 of tap pairs (broadcast) + 4 LDS.128 of map values,
                 // then 64 FFMA2.  Slot s of this thread is image 4 half + (s ^ sk); pixel pair p of slot s lives in
-                // acc01[s], acc23[s], acc01[4 + s], acc23[4 + s] for p = 0 .. 3.
+                // acc01[s], acc23[s], acc01[4 + s], acc23[4 + s] for p = 0 .. 3.  (An FFMA2 that reads two 64-bit operands
+                // from the register file -- tap pair and accumulator -- takes ~3 cycles instead of 2: a register-only loop
+                // of this operand pattern reaches 83 of 128 FMA / clk / SM; ptxas groups the FFMA2 of one
+                // tap pair so that it stays in the operand reuse slot for 3 of 4.)
                 const float *pl0 = stage + (size_t)buf * 8 * LP + (size_t)(4 * half) * LP + 8 * u8;
                 const float *pA = pl0 + sk * LP, *pB = pl0 - sk * LP;     // even / odd slots
                 float4 tp[5], mv[4];
@@ -509,8 +512,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                                 }
                             }
                         }
-                        return;
-                    }
+                    } else {
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr) {
                         const int k = k0 + 4 * tid + rr;
@@ -524,6 +526,7 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                                 tt[rr][g] = fmaf(Ku, __ldg(in + ((g < 4) ? pe.start_n : pe.start_s) + kk), tt[rr][g]);
                             }
                         }
+                    }
                     }
                 };
                 if (nexc <= kMaxExc) {
@@ -583,13 +586,13 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                                                                          tot23[4 + sl].x * P.omega, tot23[4 + sl].y * P.omega);
                     }
                 }
-                continue;
-            }
+            } else {
 #pragma unroll
             for (int g = 0; g < 8; ++g) {
                 if (g >= 4 && !south) break;
                 const float4 v = make_float4(tot01[g].x * P.omega, tot01[g].y * P.omega, tot23[g].x * P.omega, tot23[g].y * P.omega);
                 *reinterpret_cast<float4 *>(out + ((g < 4) ? start_n : start_s) + k + (g & 3) * N) = v;
+            }
             }
         }
     }

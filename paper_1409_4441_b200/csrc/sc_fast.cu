@@ -71,11 +71,12 @@ static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, 
     }
     const size_t nfull = bins.size();
     std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
+    const int Wcap = std::min(W, (run + C - 1) / C);     // warps per packed tile (< W only for small maps: runs shortened to spread over the SMs)
     std::vector<int> used(nfull, W), lsum(nfull, 0);
     for (const SubH &sb : partial) {
         size_t i = nfull;
         for (; i < bins.size(); ++i)
-            if (used[i] + sb.nw <= W && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Llimit) break;
+            if (used[i] + sb.nw <= Wcap && (int)bins[i].size() < kMaxSub && lsum[i] + sb.Lcap <= Llimit) break;
         if (i == bins.size()) { bins.emplace_back(); used.push_back(0); lsum.push_back(0); }
         bins[i].push_back(sb); used[i] += sb.nw; lsum[i] += sb.Lcap;
     }
@@ -595,7 +596,19 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int R = cd.R, W = cd.threads / 32, C = (cd.pair ? 16 : 32) * R;
             // full-width runs may be a little shorter than the CTA (last lanes idle) if that makes the
             // staged runs fit into shared memory
-            for (int shrink = 0; shrink <= W * C / 4 && !c.ok; shrink += 16) {
+            // small maps: fewer full-width tiles than SMs -> shorter runs (idle lanes, but every SM gets a tile)
+            int shrink0 = 0;
+            if (B == 1 && !std::getenv("SC_SYM_NOSPREAD")) {
+                long long base_px = 0;
+                for (int r = polar + 1; r <= 2 * N; ++r)
+                    if (!is_belt[r]) base_px += cd.mirror ? (ipof(r) + 2) / 2 : ipof(r);
+                const long long n0 = (base_px + W * C - 1) / (W * C);
+                if (n0 < fp->nsm) {
+                    const int want = std::max(2 * C, (int)(((base_px + fp->nsm - 1) / fp->nsm + 31) / 32) * 32);
+                    if (want < W * C) shrink0 = (W * C - want) & ~15;
+                }
+            }
+            for (int shrink = shrink0; shrink <= std::max(W * C / 4, shrink0) && !c.ok; shrink += 16) {
             const int run = W * C - shrink;
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int npl = cd.mirror ? 4 : 2;                      // staged planes per position (float4 of rotation images each)
