@@ -225,12 +225,16 @@ def _fma_peaks(sc):
     """FP32 FMA/s: nominal (unit counts x clock) and measured in this process (scalar FFMA, packed FFMA2)."""
     sm_max, peak_src = _sm_max_mhz()
     nominal = N_SM * LANES * sm_max * 1e6
-    m1, m2 = sc.sc_debug_fma_peak(packed=False), sc.sc_debug_fma_peak(packed=True)
+    m1, m2, m3 = sc.sc_debug_fma_peak(packed=False), sc.sc_debug_fma_peak(packed=True), sc.sc_debug_fma_peak(packed=2)
     measured = max(m1["fma_per_s"], m2["fma_per_s"])
     return nominal, measured, {
         "nominal_gfma": nominal / 1e9,
         "nominal_source": f"{N_SM} SMs x {LANES} FP32 lanes x {sm_max:.0f} MHz ({peak_src})",
         "measured_ffma_gfma": m1["fma_per_s"] / 1e9, "measured_ffma2_gfma": m2["fma_per_s"] / 1e9,
+        "measured_ffma2_kernel_operands_gfma": m3["fma_per_s"] / 1e9,
+        "kernel_operands": "FFMA2 with the accumulation's operand pattern (accumulator pair += tap pair x map value, a fresh "
+                           "64-bit accumulator and 32-bit map value every instruction, the tap pair shared by 4): what the "
+                           "register file sustains for it; the fractions of this line are against the constant-operand peak",
         "measured_source": "sc_debug_fma_peak in this run: register-only FFMA / FFMA2 loops, 2 x 1024 threads per SM, "
                            f"best of 3 launches of {m1['elapsed_ms']:.1f} / {m2['elapsed_ms']:.1f} ms (CUDA events)"}
 

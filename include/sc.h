@@ -227,7 +227,9 @@ sc_status sc_convolve_cap(sc_plan *plan, int ring_hi, const float *const *in_map
  * sc_debug_fma_peak -- measurement only: the sustained FP32 FMA rate of the current device, measured with a
  * register-only loop of independent FMA chains (packed = 0: scalar FFMA; packed = 1: FFMA2, the packed form the
  * convolution kernels accumulate with) on 2 x 1024 threads per SM, best of 3 launches of a few ms.  bench.py uses
- * it as the measured denominator of the roofline.
+ * it as the measured denominator of the roofline.  packed = 2: FFMA2 with the operand pattern of the
+ * kernels' accumulation (accumulator pair += tap pair x map value, 16 warps per SM): what the register file sustains
+ * for that pattern, reported next to the peak.  Other values: SC_ERR_INVALID_ARG.
  *   fma_per_s   HOST out: fp32 fused multiply-adds per second (an FFMA2 counts as two)
  *   elapsed_ms  HOST out (may be NULL): duration of the best launch
  * Synchronous on the legacy default stream; needs no plan.

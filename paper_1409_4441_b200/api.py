@@ -187,9 +187,10 @@ def sc_debug_neighbour_counts(plan, count_ptr, sig_ptr=0, stream=0):
 
 
 def sc_debug_fma_peak(packed=True):
-    """Measurement only: sustained FP32 FMA/s of the current device (FFMA2 loop if packed else scalar FFMA)."""
+    """Measurement only: sustained FP32 FMA/s of the current device (FFMA2 loop if packed else scalar FFMA;
+    packed = 2: FFMA2 with the operand pattern of the kernels' accumulation)."""
     v, ms = C.c_double(0), C.c_double(0)
-    _chk(lib().sc_debug_fma_peak(1 if packed else 0, C.byref(v), C.byref(ms)), "sc_debug_fma_peak")
+    _chk(lib().sc_debug_fma_peak(int(packed), C.byref(v), C.byref(ms)), "sc_debug_fma_peak")
     return dict(fma_per_s=v.value, elapsed_ms=ms.value)
 
 

@@ -43,7 +43,7 @@ struct HostGeo {
 // all_rings: also the base rings that the belt kernel normally takes (north-cap-only convolution).
 // lanes: lanes of a warp that own a group of R base pixels each (32; 16 in the lane-pair instance).
 static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, int r_hi, int r_lo, bool mirror,
-                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32) {
+                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32, int wcap = 0) {
     const int C = lanes * R;
     struct SubH { int r, k0, n, nw; int Lcap; double work; };
     auto make_sub = [&](int r, int k0, int n) {
@@ -71,7 +71,7 @@ static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, 
     }
     const size_t nfull = bins.size();
     std::stable_sort(partial.begin(), partial.end(), [](const SubH &a, const SubH &b) { return a.nw > b.nw; });
-    const int Wcap = std::min(W, (run + C - 1) / C);     // warps per packed tile (< W only for small maps: runs shortened to spread over the SMs)
+    const int Wcap = wcap > 0 ? std::min(W, wcap) : W;   // warps per packed tile (< W only for small maps: runs shortened to spread over the SMs)
     std::vector<int> used(nfull, W), lsum(nfull, 0);
     for (const SubH &sb : partial) {
         size_t i = nfull;
@@ -616,7 +616,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int Lmax = (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
             HostGeo &g = *fp->geo;
             g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;
-            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32); };
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0); };
             // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
             // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
             std::vector<SymTile> tiles;

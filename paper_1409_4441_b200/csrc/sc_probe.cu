@@ -1,7 +1,11 @@
 // sc_probe.cu -- measurement only: the sustained FP32 FMA rate of the device, the denominator of the roofline
 // that bench.py reports ("report against (i) the nominal figure and (ii) a sustained FFMA
 // microbenchmark run in the same job").  Register-only loops of independent FMA chains: scalar FFMA or packed
-// FFMA2 (fma.rn.f32x2, the instruction the convolution kernels accumulate with).
+// FFMA2 (fma.rn.f32x2, the instruction the convolution kernels accumulate with), and a third loop with the OPERAND
+// PATTERN of the kernels' accumulation -- acc_pair += tap_pair * map_value with the tap pair shared by 4 consecutive
+// FFMA2 and a fresh map value and accumulator each time: an FFMA2 that reads two 64-bit operands from the register file
+// takes ~3 issue cycles instead of 2 on this part (measured 83 against 125 FMA / clk / SM), which bounds the kernels' FMA
+// pipe utilisation below the constant-operand peak.
 #include "../../include/sc.h"
 #include <cuda_runtime.h>
 
@@ -33,6 +37,34 @@ fma_probe_kernel(float *out, int iters, float a, float b) {
     if (s == 123.456f) out[0] = s;       // never true in practice: keeps the loop alive
 }
 
+// acc[p][s] += tap[6 - 2p + i] * m[s][i]: the belt kernel's chunk (8 pixels = 4 pairs p, 4 images s, 4 positions i),
+// register only, the operands changing a little every iteration so that nothing is hoisted
+__global__ void __launch_bounds__(512, 1)
+fma_pattern_kernel(float *out, const float *in, int iters) {
+    float2 acc[16], tp[10];
+    float mv[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) { acc[j] = make_float2((float)threadIdx.x + j, (float)j - 0.5f); mv[j] = in[16 + j]; }
+#pragma unroll
+    for (int j = 0; j < 10; ++j) tp[j] = make_float2(in[j], in[j + 1]);
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int sl = 0; sl < 4; ++sl)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float2 m2 = make_float2(mv[4 * sl + i], mv[4 * sl + i]);
+#pragma unroll
+                for (int p = 0; p < 4; ++p) acc[4 * p + sl] = __ffma2_rn(tp[6 - 2 * p + i], m2, acc[4 * p + sl]);
+            }
+        tp[0].x += 1e-9f; mv[0] += 1e-9f;
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) s += acc[j].x + acc[j].y;
+    if (s == 123.456f) out[0] = s;
+}
+
 }  // namespace
 
 extern "C" sc_status sc_debug_fma_peak(int packed, double *fma_per_s, double *elapsed_ms) {
@@ -40,18 +72,22 @@ extern "C" sc_status sc_debug_fma_peak(int packed, double *fma_per_s, double *el
     int dev = 0, nsm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return SC_ERR_CUDA;
     if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) return SC_ERR_CUDA;
+    if (packed < 0 || packed > 2) return SC_ERR_INVALID_ARG;
     float *d = nullptr;
-    if (cudaMalloc((void **)&d, 4) != cudaSuccess) return SC_ERR_ALLOC;
+    if (cudaMalloc((void **)&d, 256) != cudaSuccess) return SC_ERR_ALLOC;
+    if (cudaMemset(d, 0, 256) != cudaSuccess) { cudaFree(d); return SC_ERR_CUDA; }
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     sc_status st = SC_OK;
     double best = 0.0, best_ms = 0.0;
     do {
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { st = SC_ERR_CUDA; break; }
-        const int blocks = 2 * nsm, threads = 1024, iters = 12000;       // ~ 6 ms at 128 FMA / clk / SM
-        const double fmas = (double)blocks * threads * (double)iters * 4.0 * kChains;
+        const int blocks = packed == 2 ? nsm : 2 * nsm, threads = packed == 2 ? 512 : 1024, iters = packed == 2 ? 20000 : 12000;   // ~ 6 ms at 128 FMA / clk / SM
+        const double fmas = packed == 2 ? (double)blocks * threads * (double)iters * 128.0
+                                        : (double)blocks * threads * (double)iters * 4.0 * kChains;
         for (int rep = 0; rep < 4 && st == SC_OK; ++rep) {               // first repetition = warm-up
             cudaEventRecord(e0, 0);
-            if (packed) fma_probe_kernel<true><<<blocks, threads>>>(d, iters, 1.000001f, 1e-7f);
+            if (packed == 2) fma_pattern_kernel<<<blocks, threads>>>(d + 32, d, iters);
+            else if (packed) fma_probe_kernel<true><<<blocks, threads>>>(d, iters, 1.000001f, 1e-7f);
             else fma_probe_kernel<false><<<blocks, threads>>>(d, iters, 1.000001f, 1e-7f);
             cudaEventRecord(e1, 0);
             if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { st = SC_ERR_CUDA; break; }

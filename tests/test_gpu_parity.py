@@ -926,3 +926,13 @@ def test_double_coordinate_exact_integer_sums(sc, monkeypatch):
     omega = np.float32(4.0 * np.pi / npix)
     want = (np.round(ref[0] / (4.0 * np.pi / npix)).astype(np.float32) * omega).astype(np.float32)
     np.testing.assert_array_equal(out[sel], want)
+
+
+def test_fma_peak_probe_modes(sc):
+    """sc_debug_fma_peak: scalar, packed and the kernels' operand pattern all give a plausible rate (the pattern loop
+    cannot beat the constant-operand one), other modes are refused."""
+    rates = [sc.sc_debug_fma_peak(packed=m)["fma_per_s"] for m in (0, 1, 2)]
+    assert all(1e12 < r < 1e14 for r in rates), rates
+    assert rates[2] <= 1.02 * max(rates[:2]), rates
+    with pytest.raises(sc.ScError):
+        sc.sc_debug_fma_peak(packed=3)
