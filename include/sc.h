@@ -149,6 +149,21 @@ sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uin
                                     void *cuda_stream);
 
 /*
+ * sc_neighbour_counts_static -- sc_debug_neighbour_counts for callers that must not allocate (CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, same results, asynchronous on cuda_stream for
+ * RING and NESTED plans alike, and no cudaMalloc / cudaFree or other allocating call.  The RING-ordered scratch that
+ * a NESTED plan needs (4 + 8 bytes per pixel) lives in a static device array of SC_STATIC_MAX_NPIX entries (2.25 MiB
+ * that every GPU loading the library holds until exit), so 12 nside^2 <= SC_STATIC_MAX_NPIX, i.e. nside <= 128
+ * (larger: SC_ERR_UNSUPPORTED, nothing launched).  The plan's device must be current on a device's first call
+ * (SC_ERR_INVALID_ARG otherwise): that call resolves the array's device address (cudaGetSymbolAddress), so make it
+ * outside stream capture.  All calls on a device share the array, which keeps the previous call's contents (every
+ * entry used is overwritten before it is read: nothing needs clearing); calls that OVERLAP on the GPU -- different
+ * streams, concurrent graph replays -- race on it and must be serialised by the caller.
+ */
+#define SC_STATIC_MAX_NPIX 196608
+sc_status sc_neighbour_counts_static(const sc_plan *plan, int32_t *count_dev, uint64_t *sig_dev, void *cuda_stream);
+
+/*
  * sc_debug_stats -- numbers gathered by the audit pass at plan creation (HOST outputs, may be NULL):
  *   n_uncertain   pairs whose fp32 table coordinate fell inside the guard band and were therefore
  *                 re-decided in fp64 on the device

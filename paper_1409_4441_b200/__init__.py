@@ -7,6 +7,6 @@ a CUDA device the calls raise.
 """
 from .api import (Plan, ScError, lib, sc_plan_create, sc_plan_create_zoned, sc_convolve, sc_convolve_host,  # noqa: F401
                   sc_convolve_profile, sc_plan_partition, KERNEL_NAMES, sc_band_partition, sc_convolve_band, sc_cap_rows, sc_convolve_cap,
-                  sc_plan_destroy, sc_plan_info, sc_plan_set_path, sc_debug_neighbour_counts,
+                  sc_plan_destroy, sc_plan_info, sc_plan_set_path, sc_debug_neighbour_counts, sc_neighbour_counts_static, SC_STATIC_MAX_NPIX,
                   sc_debug_stats, sc_debug_fma_peak, sc_last_launch_count, sc_plan_double_coordinate, sc_version, EXPORTS,
                   SC_ORDER_RING, SC_ORDER_NESTED, SC_PATH_AUTO, SC_PATH_GENERIC)

@@ -16,7 +16,7 @@ KERNEL_NAMES = ("generic_warp_kernel", "sym_kernel", "belt_kernel")
 EXPORTS = ("sc_plan_create", "sc_plan_create_zoned", "sc_convolve", "sc_convolve_host", "sc_convolve_profile", "sc_plan_partition",
            "sc_band_partition", "sc_convolve_band", "sc_cap_rows", "sc_convolve_cap",
            "sc_plan_destroy", "sc_plan_set_path",
-           "sc_plan_info", "sc_debug_neighbour_counts", "sc_debug_stats", "sc_debug_fma_peak", "sc_last_launch_count", "sc_plan_double_coordinate",
+           "sc_plan_info", "sc_debug_neighbour_counts", "sc_neighbour_counts_static", "sc_debug_stats", "sc_debug_fma_peak", "sc_last_launch_count", "sc_plan_double_coordinate",
            "sc_status_string", "sc_last_cuda_error", "sc_version")
 
 _lib = None
@@ -54,6 +54,7 @@ def lib():
         l.sc_plan_set_path.argtypes = [vp, i32]
         l.sc_plan_info.argtypes = [vp, vp, vp, vp, vp]
         l.sc_debug_neighbour_counts.argtypes = [vp, vp, vp, vp]
+        l.sc_neighbour_counts_static.argtypes = [vp, vp, vp, vp]
         l.sc_debug_stats.argtypes = [vp, vp, vp, vp]
         l.sc_last_launch_count.argtypes = [vp]
         l.sc_plan_double_coordinate.argtypes = [vp]
@@ -184,6 +185,16 @@ def sc_debug_stats(plan):
 def sc_debug_neighbour_counts(plan, count_ptr, sig_ptr=0, stream=0):
     _chk(lib().sc_debug_neighbour_counts(plan, C.c_void_p(int(count_ptr)), C.c_void_p(int(sig_ptr) or None),
                                          C.c_void_p(int(stream) or None)), "sc_debug_neighbour_counts")
+
+
+SC_STATIC_MAX_NPIX = 196608     # include/sc.h: entries of the static device scratch (nside <= 128)
+
+
+def sc_neighbour_counts_static(plan, count_ptr, sig_ptr=0, stream=0):
+    """sc_debug_neighbour_counts without any allocation (static device scratch; 12 nside^2 <= SC_STATIC_MAX_NPIX)."""
+    _chk(lib().sc_neighbour_counts_static(plan, C.c_void_p(int(count_ptr)), C.c_void_p(int(sig_ptr) or None),
+                                          C.c_void_p(int(stream) or None)),
+         f"sc_neighbour_counts_static (static scratch holds {SC_STATIC_MAX_NPIX} pixels: nside <= 128)")
 
 
 def sc_debug_fma_peak(packed=True):

@@ -810,3 +810,12 @@ sc_status sc_debug_neighbour_counts(const sc_plan *plan, int32_t *count_dev, uin
 }
 
 }  // extern "C"
+
+// internal accessors for sc_static.cu (the plan structure is private to this file)
+namespace sc {
+const Dev *plan_dev(const sc_plan *plan) { return plan ? &plan->dev : nullptr; }
+int plan_nested(const sc_plan *plan) { return plan ? plan->nested : 0; }
+int plan_device(const sc_plan *plan) { return plan ? plan->device : -1; }
+void note_error(const char *what, cudaError_t e) { cuda_ok(e, what); }
+void note_message(const char *msg) { g_cuda_err = msg; }
+}  // namespace sc
