@@ -313,10 +313,9 @@ belt_kernel(const Dev P, const BeltDev F, const Maps io, const int B) {
                 if constexpr (W8) {
                 // chunk g4 = 4 staged positions x 4 images: 5 LDS.128 of tap pairs (broadcast) + 4 LDS.128 of map values,
                 // then 64 FFMA2.  Slot s of this thread is image 4 half + (s ^ sk); pixel pair p of slot s lives in
-                // acc01[s], acc23[s], acc01[4 + s], acc23[4 + s] for p = 0 .. 3.  (An FFMA2 that reads two 64-bit operands
-                // from the register file -- tap pair and accumulator -- takes ~3 cycles instead of 2: a register-only loop
-                // of this operand pattern reaches 83 of 128 FMA / clk / SM; ptxas groups the FFMA2 of one
-                // tap pair so that it stays in the operand reuse slot for 3 of 4.)
+                // acc01[s], acc23[s], acc01[4 + s], acc23[4 + s] for p = 0 .. 3.  (A register-only loop of this
+                // operand pattern -- tap pair and accumulator pair from the register file, the tap pair reused by 4 FFMA2 --
+                // sustains ~105 of 128 FMA / clk / SM: sc_debug_fma_peak mode 2.)
                 const float *pl0 = stage + (size_t)buf * 8 * LP + (size_t)(4 * half) * LP + 8 * u8;
                 const float *pA = pl0 + sk * LP, *pB = pl0 - sk * LP;     // even / odd slots
                 float4 tp[5], mv[4];

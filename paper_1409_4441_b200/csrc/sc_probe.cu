@@ -2,10 +2,9 @@
 // that bench.py reports ("report against (i) the nominal figure and (ii) a sustained FFMA
 // microbenchmark run in the same job").  Register-only loops of independent FMA chains: scalar FFMA or packed
 // FFMA2 (fma.rn.f32x2, the instruction the convolution kernels accumulate with), and a third loop with the OPERAND
-// PATTERN of the kernels' accumulation -- acc_pair += tap_pair * map_value with the tap pair shared by 4 consecutive
-// FFMA2 and a fresh map value and accumulator each time: an FFMA2 that reads two 64-bit operands from the register file
-// takes ~3 issue cycles instead of 2 on this part (measured 83 against 125 FMA / clk / SM), which bounds the kernels' FMA
-// pipe utilisation below the constant-operand peak.
+// PATTERN of the belt kernel's accumulation -- acc_pair += tap_pair * map_value, the tap pair shared by 4 FFMA2 and a
+// fresh map value and accumulator pair each time: what the register file sustains for it (measured ~105 against ~125
+// FMA / clk / SM with constant operands; an arrangement whose tap pairs are not aligned register pairs drops to 83).
 #include "../../include/sc.h"
 #include <cuda_runtime.h>
 
@@ -37,27 +36,36 @@ fma_probe_kernel(float *out, int iters, float a, float b) {
     if (s == 123.456f) out[0] = s;       // never true in practice: keeps the loop alive
 }
 
-// acc[p][s] += tap[6 - 2p + i] * m[s][i]: the belt kernel's chunk (8 pixels = 4 pairs p, 4 images s, 4 positions i),
-// register only, the operands changing a little every iteration so that nothing is hoisted
+// acc[p][s] += tap[6 - 2p + i] * m[s][i]: the belt kernel's chunk (8 pixels = 4 pairs p, 4 images s, 4 positions i) with
+// its register layout -- tap pairs and map values as they come out of LDS.128 (float4), so that every tap pair is an
+// aligned register pair -- register only, the operands changing a little every iteration so that nothing is hoisted
 __global__ void __launch_bounds__(512, 1)
 fma_pattern_kernel(float *out, const float *in, int iters) {
-    float2 acc[16], tp[10];
-    float mv[16];
+    float2 acc[16];
+    float4 tp[5], mv[4];
 #pragma unroll
-    for (int j = 0; j < 16; ++j) { acc[j] = make_float2((float)threadIdx.x + j, (float)j - 0.5f); mv[j] = in[16 + j]; }
+    for (int j = 0; j < 16; ++j) acc[j] = make_float2((float)threadIdx.x + j, (float)j - 0.5f);
 #pragma unroll
-    for (int j = 0; j < 10; ++j) tp[j] = make_float2(in[j], in[j + 1]);
+    for (int j = 0; j < 5; ++j) tp[j] = make_float4(in[4 * j], in[4 * j + 1], in[4 * j + 2], in[4 * j + 3]);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) mv[j] = make_float4(in[32 + 4 * j], in[33 + 4 * j], in[34 + 4 * j], in[35 + 4 * j]);
 #pragma unroll 1
     for (int it = 0; it < iters; ++it) {
+        const float2 pwr[10] = {make_float2(tp[0].x, tp[0].y), make_float2(tp[0].z, tp[0].w), make_float2(tp[1].x, tp[1].y),
+                                make_float2(tp[1].z, tp[1].w), make_float2(tp[2].x, tp[2].y), make_float2(tp[2].z, tp[2].w),
+                                make_float2(tp[3].x, tp[3].y), make_float2(tp[3].z, tp[3].w), make_float2(tp[4].x, tp[4].y),
+                                make_float2(tp[4].z, tp[4].w)};
 #pragma unroll
-        for (int sl = 0; sl < 4; ++sl)
+        for (int sl = 0; sl < 4; ++sl) {
+            const float mm[4] = {mv[sl].x, mv[sl].y, mv[sl].z, mv[sl].w};
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                const float2 m2 = make_float2(mv[4 * sl + i], mv[4 * sl + i]);
+                const float2 m2 = make_float2(mm[i], mm[i]);
 #pragma unroll
-                for (int p = 0; p < 4; ++p) acc[4 * p + sl] = __ffma2_rn(tp[6 - 2 * p + i], m2, acc[4 * p + sl]);
+                for (int p = 0; p < 4; ++p) acc[4 * p + sl] = __ffma2_rn(pwr[6 - 2 * p + i], m2, acc[4 * p + sl]);
             }
-        tp[0].x += 1e-9f; mv[0] += 1e-9f;
+        }
+        tp[0].x += 1e-9f; mv[0].x += 1e-9f; mv[1].y += 1e-9f; mv[2].z += 1e-9f; mv[3].w += 1e-9f;
     }
     float s = 0.f;
 #pragma unroll
