@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libsc.so")
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["sc_plan.cu", "sc_generic.cu", "sc_fast.cu", "sc_sym_b1.cu", "sc_sym_bn.cu", "sc_sym_pair.cu", "sc_belt.cu", "sc_nested.cu", "sc_probe.cu", "sc_static.cu"]
+SOURCES = ["sc_plan.cu", "sc_generic.cu", "sc_fast.cu", "sc_sym_b1.cu", "sc_sym_bn.cu", "sc_sym_pl.cu", "sc_sym_pair.cu", "sc_belt.cu", "sc_nested.cu", "sc_probe.cu", "sc_static.cu"]
 HEADERS = [os.path.join(CSRC, "sc_internal.cuh"), os.path.join(CSRC, "sc_fast.cuh"), os.path.join(CSRC, "sc_sym.cuh"), os.path.join(ROOT, "include", "sc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 CFLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

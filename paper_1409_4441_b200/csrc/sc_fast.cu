@@ -43,7 +43,7 @@ struct HostGeo {
 // all_rings: also the base rings that the belt kernel normally takes (north-cap-only convolution).
 // lanes: lanes of a warp that own a group of R base pixels each (32; 16 in the lane-pair instance).
 static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, int r_hi, int r_lo, bool mirror,
-                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32, int wcap = 0) {
+                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32, int wcap = 0, int pad = 0) {
     const int C = lanes * R;
     struct SubH { int r, k0, n, nw; int Lcap; double work; };
     auto make_sub = [&](int r, int k0, int n) {
@@ -56,7 +56,7 @@ static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, 
             sb.Lcap = std::max(sb.Lcap, L);
             sb.work += (double)(2 * pe.hw + R);
         }
-        sb.Lcap = (sb.Lcap + 7) & ~7;
+        sb.Lcap = ((sb.Lcap + 7) & ~7) + pad;           // pad: alignment slack of the planar instances' bulk copies
         sb.work *= sb.nw;
         return sb;
     };
@@ -119,6 +119,7 @@ struct FastCfg {            // per batch size
     bool tot = true;              // second accumulator set (per-ring partial sums added to running totals)
     bool mirror = false;          // 16 images per pair geometry (reflection phi -> pi/2 - phi as well)
     bool pair = false;            // lane-pair instance: 16 lane pairs x R base pixels per warp
+    bool planar = false;          // planar staging by TMA bulk copies (sc_sym_pl.cu)
     std::map<std::pair<int, int>, std::pair<SymTile *, int>> band_tiles;   // (ring lo, hi) -> device tile list
     std::vector<int> ch_off, ch_lo, ch_hi;   // chunk i: tiles [ch_off[i], ch_off[i+1]), base rings ch_lo[i] .. ch_hi[i]
 };
@@ -154,7 +155,8 @@ struct FastPlan {
 static cudaError_t dispatch_sym(const FastPlan *fp, const FastCfg &c, const Dev &P, const Maps &io, int B, cudaStream_t st,
                                 const SymTile *tiles, int nt, bool south = true, bool overlap = false) {
     if (nt <= 0) return cudaSuccess;
-    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair, fp->tile_ctr, fp->pairsd, overlap};
+    const SymLaunch L{fp->pairs, tiles, nt, c.Ltot, fp->ntab_s, fp->nsm, c.threads, c.R, c.smem, c.tot, c.tmem, c.mirror, south, c.pair, fp->tile_ctr, fp->pairsd, overlap, c.planar};
+    if (c.planar) return B == 1 ? dispatch_sym_pl(L, P, io, st) : cudaErrorInvalidValue;
     if (c.pair) return B == 1 ? dispatch_sym_pair(L, P, io, st) : cudaErrorInvalidValue;
     return B == 1 ? dispatch_sym_b1(L, P, io, st) : dispatch_sym_bn(L, P, io, B, st);
 }
@@ -204,7 +206,7 @@ cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, 
         auto it = c.band_tiles.find({s_lo, s_hi});
         if (it == c.band_tiles.end()) {
             std::vector<SymTile> tiles;
-            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, c.mirror, tiles, false, c.pair ? 16 : 32);
+            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, c.mirror, tiles, false, c.pair ? 16 : 32, 0, c.planar ? kPlanarPad : 0);
             if (Lneed > c.Ltot) return cudaErrorInvalidValue;
             SymTile *d = nullptr;
             if ((e = cudaMalloc((void **)&d, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return e;
@@ -564,7 +566,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
     // Tiles are packed from sub-tiles (runs of base pixels on one ring, 32 R pixels per warp): whole
     // CTA-wide runs first, the ragged remainders of all rings are bin-packed (first fit, decreasing).
     (void)max_batch;
-    struct Cand { int threads, R; bool mirror; bool pair = false; };
+    struct Cand { int threads, R; bool mirror; bool pair = false; bool planar = false; };
     for (int B = 1; B <= kMaxB; ++B) {
         FastCfg &c = fp->cfg[B];
         std::vector<Cand> cands;
@@ -582,6 +584,10 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR")) cands.insert(cands.begin(), Cand{192, 4, true});
         // ... or 256 consumer threads x 3 base pixels: the same 768-pixel tiles with 8 consumer warps
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && !std::getenv("SC_SYM_NOR3")) cands.insert(cands.begin(), Cand{256, 3, true});
+        // ... with planar staging (one plane per image, TMA bulk copies; sc_sym_pl.cu) when the planes fit next to the table
+        if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && !std::getenv("SC_SYM_NOR3") && std::getenv("SC_SYM_PLANAR") &&
+            tab_bytes + (size_t)kSymBufH * 16 * kPlanarPlane * 4 + 512 <= (size_t)smem_optin)
+            cands.insert(cands.begin(), Cand{256, 3, true, false, true});
         // ... and as lane pairs (sc_sym_pair.cu): 32 accumulators per lane, 12 (small discs) or 8 consumer warps
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && std::getenv("SC_SYM_PAIR"))
             cands.insert(cands.begin(), mean_nb <= 700.0 ? Cand{env_int("SC_PAIR_NC", 384), 4, true, true} : Cand{256, 4, true, true});
@@ -613,10 +619,10 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             // a tile holds at most W warps, kMaxSub runs and Lmax staged positions (shared memory)
             const int npl = cd.mirror ? 4 : 2;                      // staged planes per position (float4 of rotation images each)
             const size_t stat = cd.pair ? 3072 : 512;            // static shared memory of the kernel (barriers; step records)
-            const int Lmax = (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
+            const int Lmax = cd.planar ? kPlanarPlane : (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
             HostGeo &g = *fp->geo;
             g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;
-            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0); };
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0, cd.planar ? kPlanarPad : 0); };
             // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
             // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
             std::vector<SymTile> tiles;
@@ -638,11 +644,13 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
                     }
                 }
             }
+            if (cd.planar && Ltot > kPlanarPlane) continue;
+            if (cd.planar) Ltot = kPlanarPlane;                   // the planar instances' plane length is a compile-time constant
             const size_t smem = tab_bytes + (size_t)kSymBufH * B * npl * Ltot * 16;
             if (smem + stat > (size_t)smem_optin) continue;
             c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
             c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all; c.run = run;
-            c.mirror = cd.mirror; c.pair = cd.pair;
+            c.mirror = cd.mirror; c.pair = cd.pair; c.planar = cd.planar;
             c.tmem = !cd.pair && (B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb > 700.0);      // large discs: two-level sums, totals in TMEM
             // a single accumulator set (plain fp32 running sums) only for one map and discs of at most 700 pixels
             c.tot = !(B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb <= 700.0);

@@ -62,9 +62,13 @@ struct SymLaunch {
     const PairEntD *pairsd;     // fp64 ring pairs of a Dev::hp plan
     bool overlap;               // launch with programmatic stream serialization: the CTAs may start while the previous kernel of
                                 // the stream (the belt kernel: disjoint outputs) drains; the tile counter was zeroed before that kernel
+    bool planar = false;        // planar staging by TMA bulk copies (sc_sym_pl.cu): one plane per image instead of float4-interleaved rotations
 };
 cudaError_t dispatch_sym_pair(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
 cudaError_t dispatch_sym_b1(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
+cudaError_t dispatch_sym_pl(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st);
+constexpr int kPlanarPlane = 784;   // floats per image plane of the planar instances (kLp in sc_sym.cuh)
+constexpr int kPlanarPad = 8;       // extra staged floats per run: 0-3 in front (alignment in the ring), rounded up to 4 behind
 cudaError_t dispatch_sym_bn(const SymLaunch &L, const Dev &P, const Maps &io, int B, cudaStream_t st);
 
 constexpr int kMaxExc = 32;      // uncertain taps per belt tile that can be listed (more -> rescan)

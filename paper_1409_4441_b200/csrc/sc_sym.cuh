@@ -105,6 +105,9 @@ constexpr int kSymBuf = 2;        // stage buffers
 #ifndef SC_R3_PIPE
 #define SC_R3_PIPE 0
 #endif
+#ifndef SC_PLN_UNROLL
+#define SC_PLN_UNROLL 2          // positions per iteration of the planar instances' main loop (2 or 4)
+#endif
 __host__ __device__ constexpr int sym_nprod(int NC) { return (NC == 192 && SC_L192 == 1) ? 64 : 128; }
 // SC_L192 == 0 (A/B layout): warps 0-5 = consumers, 6-7 = idle (they exit after the register hand-over of their
 // warpgroup: setmaxnreg works on whole warpgroups), 8-11 = producers.
@@ -126,6 +129,20 @@ template <int R, int B, int NPL> struct SymLd { float2 el[R]; float4 mv[B][NPL];
 // get equal shares of the work-sorted tile list without a global counter.
 __device__ __forceinline__ int snake_tile(int row, int G, int bid) { return row * G + ((row & 1) ? G - 1 - bid : bid); }
 
+// 4 bytes at shared address a + IMM (IMM: compile-time plane offset, folded into the instruction)
+template <int IMM> __device__ __forceinline__ float lds32(unsigned a) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(IMM));
+    return v;
+}
+
+// Planar staging (template flag PLN; R = 3, one map): every image has a plane of its own (4 NPL planes of kLp floats per
+// stage buffer), filled by TMA bulk copies of 16-byte-aligned pieces of the input rings -- the run of an image starts 0-3
+// floats into its plane (its alignment in the ring; ring starts and lengths are multiples of 4 pixels), the reflected
+// images are staged in ring order and read backwards.  The consumers read one float per image and position (LDS.32:
+// lanes 3 positions apart hit 32 different banks) instead of one float4 per plane of 4 interleaved rotation images.
+constexpr int kLp = kPlanarPlane;          // floats per plane: 2 buffers x 16 planes x 784 x 4 B = 98 KB next to the 128 KB table
+
 __device__ __forceinline__ float4 lds128(unsigned a) {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
@@ -139,16 +156,20 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 // discs of thousands of pixels, costs as many registers again).
 // Z: two-zone table (lookup at tau(t), R11).  TM: the second accumulator set lives in tensor memory.
 // HP: table coordinate in fp64 (Dev::hp, steep tables), split into cell + position in the cell; cell-local table.
-template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR, bool HP = false>
+template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR, bool HP = false, bool PLN = false>
 __global__ void __launch_bounds__(sym_threads(NC), 1)
 sym_kernel(const Dev P, const FastDev F, const Maps io) {
     static_assert(!(HP && Z), "the fp64 coordinate is not combined with the two-zone table");
+    static_assert(!PLN || (B == 1 && (R == 3 || R == 1)), "planar staging: one map, lanes 3 positions (or 1) apart");
     static_assert(R >= 1 && R <= 4, "R");
     constexpr int RP = (R + 1) / 2;                      // pixel pairs per thread
     constexpr int NPROD = sym_nprod(NC), PROD0 = sym_prod0(NC);
     constexpr int NPL = sym_planes(SOUTH, MIRROR);       // staged planes per position, 4 rotation images each
     constexpr int G = 2 * NPL;                           // float2 accumulators per base pixel and map
     constexpr int TMC = sym_tmem_cols(NC, R * G * 2);
+    constexpr int NPD = SOUTH ? 2 : 1;                   // planes of direct images (the others: reflected)
+    constexpr int NTASK = PLN ? 4 * NPL * kMaxSub : 0;   // planar staging: bulk-copy tasks (sub-tile, image) = producer threads that arrive
+    static_assert(NTASK <= NPROD, "one producer thread per (sub-tile, image)");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float2 *tab = reinterpret_cast<float2 *>(smem_raw);
     const unsigned stage_sh = smem_u32(smem_raw + (((size_t)F.ntab_s * 8 + 127) & ~(size_t)127));
@@ -170,7 +191,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     if (!BULK)
         for (int i = tid; i < F.ntab_s; i += blockDim.x) tab[i] = P.tabh[i];
     if (tid == 0) {
-        for (int i = 0; i < kSymBuf; ++i) { mbar_init(&full_bar[i], NPROD); mbar_init(&empty_bar[i], NC / 32); }
+        for (int i = 0; i < kSymBuf; ++i) { mbar_init(&full_bar[i], PLN ? NTASK : NPROD); mbar_init(&empty_bar[i], NC / 32); }
         if (BULK) mbar_init(&tab_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         if (BULK) {
@@ -233,7 +254,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             const int tile = *(volatile int *)&s_tile[n & 3];
             if (tile < 0) {                              // no more tiles: wake the consumers with one empty step
                 mbar_wait_sleep(&empty_bar[it % kSymBuf], ((it / kSymBuf) & 1u) ^ 1u);
-                cp_async_mbar_arrive(&full_bar[it % kSymBuf]);
+                if (!PLN) cp_async_mbar_arrive(&full_bar[it % kSymBuf]);
+                else if (pt < NTASK) mbar_arrive(&full_bar[it % kSymBuf]);
                 break;
             }
             const SymTile *tl = F.tiles + tile;
@@ -242,6 +264,33 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             for (int step = 0; step < nsteps; ++step, ++it) {
                 const int buf = it % kSymBuf;
                 asm volatile("bar.sync 1, %0;" ::"n"(NPROD) : "memory");        // this step's runs are in s_run[it & 1]
+                if constexpr (PLN) {
+                    // one producer thread per (sub-tile, image): the image's run as one or two (wrap) 16-byte-aligned bulk copies
+                    mbar_wait_sleep(&empty_bar[buf], ((it / kSymBuf) & 1u) ^ 1u);   // every consumer warp released it
+                    if (pt < NTASK) {
+                        const int s = pt / (4 * NPL), img = pt % (4 * NPL), pl = img >> 2, mr = img & 3;
+                        const int4 ra = s_run[it & 1][s][0], rb = s_run[it & 1][s][1];
+                        const int L = ra.z, nq = ra.w;
+                        unsigned long long *bar = &full_bar[buf];
+                        if (L > 0 && !(F.dbg & 2)) {
+                            int first = (pl < NPD ? ra.x : ra.y - (L - 1)) + mr * (nq >> 2);   // first pixel in ring order
+                            first %= nq; if (first < 0) first += nq;
+                            const int a = first & ~3, n4 = ((first & 3) + L + 3) & ~3;            // aligned piece: pixels a .. a + n4
+                            const bool sth = SOUTH && ((pl < NPD ? pl : pl - NPD) & 1);
+                            const float *ring = io.in[0] + (sth ? rb.y : rb.x);
+                            float *dst = reinterpret_cast<float *>(smem_raw + (((size_t)F.ntab_s * 8 + 127) & ~(size_t)127)) +
+                                         (size_t)(buf * 4 * NPL + img) * kLp + rb.z;
+                            const int n1 = min(n4, nq - a);
+                            mbar_expect_tx(bar, (unsigned)n4 * 4u);
+                            tma_load_1d(dst, ring + a, (unsigned)n1 * 4u, bar);
+                            if (n1 < n4) tma_load_1d(dst + n1, ring, (unsigned)(n4 - n1) * 4u, bar);
+                        } else {
+                            mbar_arrive(bar);
+                        }
+                    }
+                    if (pt < kMaxSub && step + 1 < nsteps) run_of(tl, step + 1, pt, (it + 1) & 1);
+                    continue;
+                }
                 // The runs to stage for this step (one per sub-tile) were worked out by producer threads 0 .. kMaxSub - 1 during
                 // the PREVIOUS step (run_of below) and handed over through s_run: nobody walks the dependent loads
                 // tile -> ring pair in every thread, and they are off the critical path.
@@ -405,9 +454,38 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     asm volatile("mov.u32 %0, %0;" : "+r"(pn[b]));      // one register, not re-derived per position
                 }
                 const unsigned plane = (unsigned)Ltot * 16u;
+                // planar staging: shared address of position 0 of the 4 direct rotation images (north plane; position i at
+                // +4 i) and of the 4 reflected ones (position i at -4 i); the southern planes lie 4 kLp floats further
+                unsigned ad[PLN ? 4 : 1], am[PLN ? 4 : 1];
+                if constexpr (PLN) {
+                    const int Lrun = div_fast((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) + pe.hw + R - w0;
+                    const unsigned b0 = stage_sh + (unsigned)(buf * 4 * NPL * kLp + me.soff) * 4u;
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        const int fd = w0 + m * pe.ipq;                                   // first staged pixel (mod 4 = mod-nq value mod 4)
+                        const int fm = pe.ipq - 1 + pe.shq - w0 + m * pe.ipq - (Lrun - 1);   // reflected run: first pixel in ring order
+                        ad[m] = b0 + (unsigned)(m * kLp + (fd & 3)) * 4u;
+                        am[m] = b0 + (unsigned)((4 * NPD + m) * kLp + (fm & 3) + Lrun - 1) * 4u;
+                    }
+                }
+                // the 4 rotation images of plane pl at staged position pos (planar: ad / am point at position pos - U, with
+                // U a compile-time constant: the unrolled main loop advances the 8 addresses once per kUn positions)
+                auto ldmap = [&](int b, auto PLc, int pos, auto Uc) -> float4 {
+                    constexpr int pl = decltype(PLc)::value;
+                    if constexpr (PLN) {
+                        constexpr int U = decltype(Uc)::value;
+                        constexpr int off = (pl < NPD ? pl : pl - NPD) * 4 * kLp * 4;
+                        if constexpr (pl < NPD)
+                            return make_float4(lds32<off + 4 * U>(ad[0]), lds32<off + 4 * U>(ad[1]), lds32<off + 4 * U>(ad[2]), lds32<off + 4 * U>(ad[3]));
+                        else
+                            return make_float4(lds32<off - 4 * U>(am[0]), lds32<off - 4 * U>(am[1]), lds32<off - 4 * U>(am[2]), lds32<off - 4 * U>(am[3]));
+                    } else {
+                        return lds128(pn[b] + 16u * (unsigned)slot_of_pos<R>(pos) + pl * plane);
+                    }
+                };
 
                 // last table cell or the zero cell after it (rare): exact decision where needed
-                auto slow = [&](int rr, float tpv, unsigned &cb, int pos) {
+                auto slow = [&](int rr, float tpv, unsigned &cb, int pos, auto Uc) {
                     const float t = tpv + 0.5f;
                     if (t >= tmax - eps) {
                         if (t <= tmax + eps) {                   // decide in fp64, image by image
@@ -421,16 +499,19 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                                 const float Ku = fmaf(xk, el.y, el.x);
 #pragma unroll
                                 for (int b = 0; b < B; ++b) {
-                                    const unsigned a = pn[b] + 16u * (unsigned)slot_of_pos<R>(pos);
-#pragma unroll
-                                    for (int pl = 0; pl < NPL; ++pl) {
-                                        const float4 mq = lds128(a + pl * plane);
-                                        const unsigned mk = mask >> (4 * pl);
-                                        if (mk & 1u) acc[rr][b][2 * pl].x = fmaf(Ku, mq.x, acc[rr][b][2 * pl].x);
-                                        if (mk & 2u) acc[rr][b][2 * pl].y = fmaf(Ku, mq.y, acc[rr][b][2 * pl].y);
-                                        if (mk & 4u) acc[rr][b][2 * pl + 1].x = fmaf(Ku, mq.z, acc[rr][b][2 * pl + 1].x);
-                                        if (mk & 8u) acc[rr][b][2 * pl + 1].y = fmaf(Ku, mq.w, acc[rr][b][2 * pl + 1].y);
-                                    }
+                                    auto one = [&](auto PLc) {
+                                        constexpr int pl = decltype(PLc)::value;
+                                        if constexpr (pl < NPL) {
+                                            const float4 mq = ldmap(b, PLc, pos, Uc);
+                                            const unsigned mk = mask >> (4 * pl);
+                                            if (mk & 1u) acc[rr][b][2 * pl].x = fmaf(Ku, mq.x, acc[rr][b][2 * pl].x);
+                                            if (mk & 2u) acc[rr][b][2 * pl].y = fmaf(Ku, mq.y, acc[rr][b][2 * pl].y);
+                                            if (mk & 4u) acc[rr][b][2 * pl + 1].x = fmaf(Ku, mq.z, acc[rr][b][2 * pl + 1].x);
+                                            if (mk & 8u) acc[rr][b][2 * pl + 1].y = fmaf(Ku, mq.w, acc[rr][b][2 * pl + 1].y);
+                                        }
+                                    };
+                                    one(std::integral_constant<int, 0>{}); one(std::integral_constant<int, 1>{});
+                                    one(std::integral_constant<int, 2>{}); one(std::integral_constant<int, 3>{});
                                 }
                             }
                         }
@@ -459,7 +540,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 //         exact fp64 decisions for the rare cells next to theta_max (slow);
                 //   load: the table cells (one LDS.64 gather per pixel) and the map values of this position;
                 //   fma:  K = a + t b and the accumulation into the images.
-                auto geom = [&](int pos, auto MASK, SymGeo<R> &ge) {
+                auto geom = [&](int pos, auto MASK, SymGeo<R> &ge, auto Uc) {
                     float *gt = ge.t;
                     unsigned *gc = ge.c;
                     constexpr int mask = decltype(MASK)::value;
@@ -515,11 +596,11 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     if (mn < 2u) {
 #pragma unroll
                         for (int rr = 0; rr < R; ++rr)
-                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], gc[rr], pos);
+                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], gc[rr], pos, Uc);
                     }
                     jf = __fadd2_rn(jf, f2(1.0f));
                 };
-                auto load = [&](int pos, auto MASK, const SymGeo<R> &ge, SymLd<R, B, NPL> &ld) {
+                auto load = [&](int pos, auto MASK, const SymGeo<R> &ge, SymLd<R, B, NPL> &ld, auto Uc) {
                     const unsigned *gc = ge.c;
                     float2 *el = ld.el;
                     float4 (*mv)[NPL] = ld.mv;
@@ -529,11 +610,15 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         if (!((mask >> rr) & 1)) continue;          // tab[gc - kMagicBits], one LEA for the address
                         asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(el[rr].x), "=f"(el[rr].y) : "r"(tab_sh + gc[rr] * 8u));
                     }
-                    const unsigned so = 16u * (unsigned)slot_of_pos<R>(pos);
 #pragma unroll
-                    for (int b = 0; b < B; ++b)
-#pragma unroll
-                        for (int pl = 0; pl < NPL; ++pl) mv[b][pl] = lds128(pn[b] + so + pl * plane);
+                    for (int b = 0; b < B; ++b) {
+                        mv[b][0] = ldmap(b, std::integral_constant<int, 0>{}, pos, Uc);
+                        if constexpr (NPL > 1) mv[b][1] = ldmap(b, std::integral_constant<int, 1>{}, pos, Uc);
+                        if constexpr (NPL > 2) {
+                            mv[b][2] = ldmap(b, std::integral_constant<int, 2>{}, pos, Uc);
+                            mv[b][3] = ldmap(b, std::integral_constant<int, 3>{}, pos, Uc);
+                        }
+                    }
                 };
                 auto fma = [&](auto MASK, const SymGeo<R> &ge, const SymLd<R, B, NPL> &ld) {
                     const float *gt = ge.t;
@@ -555,14 +640,33 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 };
                 SymGeo<R> geA, geB;
                 SymLd<R, B, NPL> ldA, ldB;
-                auto body = [&](int pos, auto MASK) {             // one position, not pipelined (window edges)
-                    geom(pos, MASK, geA);
-                    load(pos, MASK, geA, ldA);
+                const auto U0 = std::integral_constant<int, 0>{};
+                auto bodyu = [&](int pos, auto MASK, auto Uc) {   // one position, not pipelined
+                    geom(pos, MASK, geA, Uc);
+                    load(pos, MASK, geA, ldA, Uc);
                     fma(MASK, geA, ldA);
+                };
+                auto adv = [&](int n) {                           // planar: the image addresses move on by n positions
+                    if constexpr (PLN) {
+#pragma unroll
+                        for (int m = 0; m < 4; ++m) { ad[m] += 4u * (unsigned)n; am[m] -= 4u * (unsigned)n; }
+                    }
+                };
+                auto body = [&](int pos, auto MASK) {             // (window edges)
+                    bodyu(pos, MASK, U0);
+                    adv(1);
                 };
                 constexpr int kAll = (1 << R) - 1;
                 const auto ALL = std::integral_constant<int, kAll>{};
                 int pos = pos0, plast = pend;
+                if constexpr (PLN) {                              // ad / am: position pos0 from here on
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        ad[m] += 4u * (unsigned)pos0; am[m] -= 4u * (unsigned)pos0;
+                        asm volatile("mov.u32 %0, %0;" : "+r"(ad[m]));      // registers, not re-derived per position
+                        asm volatile("mov.u32 %0, %0;" : "+r"(am[m]));
+                    }
+                }
                 const bool peel = R > 1 && 2 * pe.hw >= R - 2;       // first and last R - 1 positions do not overlap
                 if (peel) {
                     body(pos++, std::integral_constant<int, 1>{});
@@ -575,22 +679,36 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 // number of positions is the same for all lanes (2 hw + R - 2 (R - 1) or 2 hw + R).
                 int left = plast - pos + 1;
                 constexpr bool PIPE = NC == 192 || (R == 3 && SC_R3_PIPE);                     // only the 6-warp instance needs it (elsewhere: spills, slower)
-                if (!PIPE) {
+                if (PLN) {
+                    constexpr int kUn = SC_PLN_UNROLL;
+#pragma unroll 1
+                    for (; pos + kUn - 1 <= plast; pos += kUn) {
+                        bodyu(pos, ALL, U0);
+                        bodyu(pos + 1, ALL, std::integral_constant<int, 1>{});
+                        if constexpr (kUn == 4) {
+                            bodyu(pos + 2, ALL, std::integral_constant<int, 2>{});
+                            bodyu(pos + 3, ALL, std::integral_constant<int, 3>{});
+                        }
+                        adv(kUn);
+                    }
+#pragma unroll 1
+                    for (; pos <= plast; ++pos) body(pos, ALL);
+                } else if (!PIPE) {
 #pragma unroll 2
                     for (; pos <= plast; ++pos) body(pos, ALL);
                 } else if (left > 0) {
-                    geom(pos, ALL, geA);
-                    load(pos, ALL, geA, ldA);
-                    if (left > 1) geom(pos + 1, ALL, geB);
+                    geom(pos, ALL, geA, U0);
+                    load(pos, ALL, geA, ldA, U0);
+                    if (left > 1) geom(pos + 1, ALL, geB, U0);
                     while (true) {
-                        if (left > 1) load(pos + 1, ALL, geB, ldB);
+                        if (left > 1) load(pos + 1, ALL, geB, ldB, U0);
                         fma(ALL, geA, ldA);
-                        if (left > 2) geom(pos + 2, ALL, geA);
+                        if (left > 2) geom(pos + 2, ALL, geA, U0);
                         ++pos;
                         if (--left == 0) break;
-                        if (left > 1) load(pos + 1, ALL, geA, ldA);
+                        if (left > 1) load(pos + 1, ALL, geA, ldA, U0);
                         fma(ALL, geB, ldB);
-                        if (left > 2) geom(pos + 2, ALL, geB);
+                        if (left > 2) geom(pos + 2, ALL, geB, U0);
                         ++pos;
                         if (--left == 0) break;
                     }
@@ -682,12 +800,12 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     }
 }
 
-template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR, bool HP = false>
+template <int B, int R, int NC, bool TOT, bool Z, bool TM, bool SOUTH, bool MIRROR, bool HP = false, bool PLN = false>
 static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, cudaStream_t st) {
     const char *dbg = std::getenv("SC_DBG");
     FastDev F{L.pairs, L.tiles, L.ntiles, L.Ltot, L.ntab_s, dbg ? std::atoi(dbg) : 0, L.pairsd, L.tile_ctr};
     static bool attr_done[64] = {};
-    cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP>, attr_done);
+    cudaError_t e = ensure_max_smem(sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP, PLN>, attr_done);
     if (e != cudaSuccess) return e;
     const int grid = std::min(L.nsm, L.ntiles);
     if (grid <= 0) return cudaSuccess;
@@ -698,10 +816,10 @@ static cudaError_t launch_sym(const SymLaunch &L, const Dev &P, const Maps &io, 
         at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at.val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = &at; cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP>, P, F, io);
+        return cudaLaunchKernelEx(&cfg, sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP, PLN>, P, F, io);
     }
     if ((e = cudaMemsetAsync(L.tile_ctr, 0, sizeof(int), st)) != cudaSuccess) return e;      // the launch's tile counter
-    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
+    sym_kernel<B, R, NC, TOT, Z, TM, SOUTH, MIRROR, HP, PLN><<<grid, sym_threads(NC), L.smem, st>>>(P, F, io);
     return cudaGetLastError();
 }
 
