@@ -106,7 +106,7 @@ constexpr int kSymBuf = 2;        // stage buffers
 #define SC_R3_PIPE 0
 #endif
 #ifndef SC_PLN_UNROLL
-#define SC_PLN_UNROLL 2          // positions per iteration of the planar instances' main loop (2 or 4)
+#define SC_PLN_UNROLL 2          // positions per iteration of the planar instances' main loop (2 or 4; 4 measured slower)
 #endif
 __host__ __device__ constexpr int sym_nprod(int NC) { return (NC == 192 && SC_L192 == 1) ? 64 : 128; }
 // SC_L192 == 0 (A/B layout): warps 0-5 = consumers, 6-7 = idle (they exit after the register hand-over of their

@@ -289,6 +289,24 @@ def test_exact_integer_sums_fast_kernels(sc, nside, theta_am, ntab, B):
         assert bad.size == 0, (part, sel[bad[:10]], out[b][sel][bad[:10]], want[bad[:10]])
 
 
+@pytest.mark.parametrize("nside,theta_am,ntab", [(1024, 30, 8192), (1024, 40, 4096), (2048, 20, 16384)])
+def test_sym_staging_layouts_agree(sc, nside, theta_am, ntab, monkeypatch):
+    """The 16-image sym kernel stages its input runs either as one plane per image by TMA bulk copies (the default,
+    sc_sym_pl.cu) or as float4-interleaved rotation images by 4-byte cp.async (SC_SYM_NOPLANAR): the same pair loop in
+    the same order, so the outputs agree bit for bit."""
+    theta = theta_am * gen.ARCMIN
+    npix = 12 * nside * nside
+    rng = np.random.default_rng(nside + theta_am)
+    m = rng.standard_normal(npix).astype(np.float32)
+    T = np.exp(-np.linspace(4.0, 0.0, ntab))
+    with sc.Plan(nside, T, theta, 1) as plan:
+        a = _gpu_convolve(sc, plan, [m])[0]
+    monkeypatch.setenv("SC_SYM_NOPLANAR", "1")
+    with sc.Plan(nside, T, theta, 1) as plan:
+        b = _gpu_convolve(sc, plan, [m])[0]
+    np.testing.assert_array_equal(a, b)
+
+
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("nside,theta_deg,ntab", [(1, 60.0, 17), (2, 50.0, 2), (3, 89.9, 33), (5, 30.0, 100),
                                                   (8, 75.0, 257), (16, 13.6, 1000), (32, 0.5, 64),
