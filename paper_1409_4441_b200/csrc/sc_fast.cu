@@ -52,7 +52,7 @@ static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, 
         const int klast = k0 + n - 1;
         for (const PairEnt &pe : g.per_ring[r]) {
             const int w0 = ((2 * k0 + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) - pe.hw;
-            const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0;
+            const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0 + (pad > 0 ? 2 * pe.ex : 0);
             sb.Lcap = std::max(sb.Lcap, L);
             sb.work += (double)(2 * pe.hw + R);
         }
@@ -387,7 +387,11 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if ((hw + 1 + Rmax) * dphi > dmax) ok = false;
             PairEnt e;
             e.A = (float)(A64 * P.scale - 0.5);
-            e.c1 = (float)(Bs / 2.0); e.c2 = (float)(-Bs / 24.0); e.c3 = (float)(Bs / 720.0); e.c4 = (float)(-Bs / 40320.0); e.pad_ = 0;
+            e.c1 = (float)(Bs / 2.0); e.c2 = (float)(-Bs / 24.0); e.c3 = (float)(Bs / 720.0); e.c4 = (float)(-Bs / 40320.0);
+            // lane skew of the planar sym instances (3 base pixels per lane): drift of 32 lanes against this ring, + 1;
+            // not worth it beyond 8 positions (rings next to the pole), not possible if the longer window would wrap
+            e.ex = ipq == ip ? 0 : (int)std::ceil(31.0 * 3.0 * rho1) + 1;
+            if (e.ex > 8 || ipq + 2 * hw + 2 * Rmax + 4 + 2 * e.ex >= 4 * ipq) e.ex = 0;
             e.dphi = (float)dphi;
             e.cdc = (float)(M_PI / (4.0 * (double)ip * (double)ipq));
             e.rq = rq; e.hw = hw; e.ipq = ipq; e.shq = shof(rq);

@@ -16,7 +16,8 @@ struct PairEnt {            // uniform per (base ring, input ring); 56 bytes
     int rq, hw, ipq, shq;   // input ring, half window (pixels), pixels per quadrant, shift flag
     int start_n, start_s;   // first pixel of the input ring and of its southern mirror
     float c4;               // B * scale * (-1/40320): fourth term of 1 - cos d
-    int pad_;
+    int ex;                 // planar sym instances: positions staged beyond the window on both sides (>= the drift of 32 lanes
+                            // 3 base pixels apart against this ring's pixel spacing); 0 = no lane skew on this ring pair
 };
 
 // The same ring pair in fp64 for plans with Dev::hp (steep tables): t = A + Bs (1 - cos d), d = (integer offset) cdc + j dphi

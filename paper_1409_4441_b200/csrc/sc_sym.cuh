@@ -234,8 +234,9 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
                 const int nq = 4 * ipq;
                 const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
-                const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw;
-                const int L = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R - w0;
+                const int ex = PLN ? __ldg(&pe->ex) : 0;      // planar: extra positions on both sides (lane skew of the consumers)
+                const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw - ex;
+                const int L = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R + ex - w0;
                 int k = w0 + nq;                          // in [0, 2 nq): w0 >= -hw - 1 > -nq
                 if (k >= nq) k -= nq;
                 // mirror image of position i: pixel ipq - 1 + shq - (w0 + i), walking backwards
@@ -430,7 +431,8 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             if (step + 1 < me.ne) pe_next = F.pairs[me.e0 + step + 1];       // prefetch under the pair loop
             mbar_wait(&full_bar[buf], (it / kSymBuf) & 1u);
             if (active && step < me.ne && !(F.dbg & 1)) {
-                const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw;
+                const int ex = PLN ? pe.ex : 0;
+                const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw - ex;
                 int rem;
                 const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
                 // azimuth of input pixel kc + j seen from base pixel ka + rr:  d = dcr[rr] + j dphi'
@@ -458,7 +460,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 // +4 i) and of the 4 reflected ones (position i at -4 i); the southern planes lie 4 kLp floats further
                 unsigned ad[PLN ? 4 : 1], am[PLN ? 4 : 1];
                 if constexpr (PLN) {
-                    const int Lrun = div_fast((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) + pe.hw + R - w0;
+                    const int Lrun = div_fast((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) + pe.hw + R + ex - w0;
                     const unsigned b0 = stage_sh + (unsigned)(buf * 4 * NPL * kLp + me.soff) * 4u;
 #pragma unroll
                     for (int m = 0; m < 4; ++m) {
@@ -527,8 +529,23 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 float2 dc2[RP];
 #pragma unroll
                 for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[2 * h + 1 < R ? 2 * h + 1 : 2 * h]);
-                float2 jf = f2((float)(-pe.hw));
-                const int pos0 = i0 - pe.hw, pend = i0 + pe.hw + R - 1;
+                // Planar staging, lane skew: on an input ring with another pixel count the lanes' positions, R apart on the base
+                // ring, drift apart by up to ex and their 4-byte loads would collide in the banks.  A lane whose position is
+                // `skew` ahead of the grid (first valid lane's position + R per lane, shifted to the smallest) starts its walk
+                // `skew` positions early and all lanes walk 2 hw + R + wd positions (wd = the largest skew of the warp): at
+                // every step the valid lanes are exactly R positions apart.  The extra positions lie outside the disc (weight
+                // 0) and inside the staged run (extended by ex on both sides).
+                int skew = 0, wd = 0;
+                if (PLN && ex > 0) {
+                    const bool valid = kmine <= klast;
+                    const int q = i0 - R * lane;
+                    const int mn = __reduce_min_sync(0xFFFFFFFFu, valid ? q : 0x7FFFFFFF);
+                    const int mx = __reduce_max_sync(0xFFFFFFFFu, valid ? q : (int)0x80000000);
+                    skew = valid ? q - mn : 0;
+                    wd = mx - mn;
+                }
+                float2 jf = f2((float)(-pe.hw - skew));
+                const int pos0 = i0 - pe.hw - skew, pend = i0 + pe.hw + R - 1 + wd - skew;
                 // One window position for the pixels rr in MASK (compile time).  The window of the thread is the
                 // union of its R pixels' windows, which are one position apart: pixel rr can only be inside the
                 // disc at positions pos0 + rr .. pend - (R - 1 - rr) (host: hw = floor(H / dphi' + 1/2 + 3 rho1),

@@ -292,19 +292,27 @@ def test_exact_integer_sums_fast_kernels(sc, nside, theta_am, ntab, B):
 @pytest.mark.parametrize("nside,theta_am,ntab", [(1024, 30, 8192), (1024, 40, 4096), (2048, 20, 16384)])
 def test_sym_staging_layouts_agree(sc, nside, theta_am, ntab, monkeypatch):
     """The 16-image sym kernel stages its input runs either as one plane per image by TMA bulk copies (the default,
-    sc_sym_pl.cu) or as float4-interleaved rotation images by 4-byte cp.async (SC_SYM_NOPLANAR): the same pair loop in
-    the same order, so the outputs agree bit for bit."""
+    sc_sym_pl.cu; lanes skewed so that their 4-byte loads stay 3 positions apart) or as float4-interleaved rotation
+    images by 4-byte cp.async (SC_SYM_NOPLANAR).  Same pairs, same weights up to the fp32 rounding of the azimuth (the
+    tilings differ, so a pixel's offset is split differently between the integer part and j dphi'): the outputs agree
+    to fp32 rounding, and with K == 1 and integer maps bit for bit."""
     theta = theta_am * gen.ARCMIN
     npix = 12 * nside * nside
     rng = np.random.default_rng(nside + theta_am)
     m = rng.standard_normal(npix).astype(np.float32)
+    mi = rng.integers(-8, 9, size=npix).astype(np.float32)
     T = np.exp(-np.linspace(4.0, 0.0, ntab))
-    with sc.Plan(nside, T, theta, 1) as plan:
-        a = _gpu_convolve(sc, plan, [m])[0]
-    monkeypatch.setenv("SC_SYM_NOPLANAR", "1")
-    with sc.Plan(nside, T, theta, 1) as plan:
-        b = _gpu_convolve(sc, plan, [m])[0]
-    np.testing.assert_array_equal(a, b)
+    res = []
+    for noplanar in (False, True):
+        if noplanar:
+            monkeypatch.setenv("SC_SYM_NOPLANAR", "1")
+        with sc.Plan(nside, T, theta, 1) as plan:
+            a = _gpu_convolve(sc, plan, [m])[0]
+        with sc.Plan(nside, np.ones(ntab), theta, 1) as plan:
+            ai = _gpu_convolve(sc, plan, [mi])[0]
+        res.append((a, ai))
+    np.testing.assert_array_equal(res[0][1], res[1][1])
+    assert np.max(np.abs(res[0][0] - res[1][0])) <= 2e-6 * np.max(np.abs(res[0][0]))
 
 
 @pytest.mark.parametrize("path", PATHS)
