@@ -105,6 +105,9 @@ constexpr int kSymBuf = 2;        // stage buffers
 #ifndef SC_R3_PIPE
 #define SC_R3_PIPE 0
 #endif
+#ifndef SC_PLN_BATCH
+#define SC_PLN_BATCH 1           // planar instances: two positions per straight-line block (one branch for the exact path)
+#endif
 #ifndef SC_PLN_UNROLL
 #define SC_PLN_UNROLL 2          // positions per iteration of the planar instances' main loop (2 or 4; 4 measured slower)
 #endif
@@ -122,7 +125,8 @@ __host__ __device__ constexpr int sym_tmem_cols(int NC, int per_thread) {
 
 // Per-position state of the pair loop: lookup coordinate - 1/2 and table cell bits of the R pixels (geometry stage),
 // table cells and map values (load stage)
-template <int R> struct SymGeo { float t[2 * ((R + 1) / 2)]; unsigned c[2 * ((R + 1) / 2)]; };
+// (tp, cb: coordinate - 1/2 and cell bits before the two-zone / fp64 / clamping steps, for the exact path)
+template <int R> struct SymGeo { float t[2 * ((R + 1) / 2)]; unsigned c[2 * ((R + 1) / 2)]; float tp[2 * ((R + 1) / 2)]; unsigned cb[2 * ((R + 1) / 2)]; };
 template <int R, int B, int NPL> struct SymLd { float2 el[R]; float4 mv[B][NPL]; };
 
 // Tile n of this CTA: rows of gridDim.x tiles, alternate rows reversed ("snake") so that the CTAs
@@ -557,12 +561,14 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 //         exact fp64 decisions for the rare cells next to theta_max (slow);
                 //   load: the table cells (one LDS.64 gather per pixel) and the map values of this position;
                 //   fma:  K = a + t b and the accumulation into the images.
-                auto geom = [&](int pos, auto MASK, SymGeo<R> &ge, auto Uc) {
+                // (geomA: the arithmetic, returns the distance of the nearest cell to the last table cell -- < 2 means some pixel
+                // needs geomS, the exact decisions; two positions can run geomA back to back before one shared branch)
+                auto geomA = [&](auto MASK, SymGeo<R> &ge) -> unsigned {
                     float *gt = ge.t;
                     unsigned *gc = ge.c;
                     constexpr int mask = decltype(MASK)::value;
-                    float tp[2 * RP];
-                    unsigned cb[2 * RP];
+                    float *tp = ge.tp;
+                    unsigned *cb = ge.cb;
 #pragma unroll
                     for (int h = 0; h < RP; ++h) {
                         if (!((mask >> (2 * h)) & 3)) continue;
@@ -610,12 +616,17 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                     for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) mn = min(mn, cb[rr] - thresh);
 #pragma unroll
                     for (int rr = 0; rr < R; ++rr) if ((mask >> rr) & 1) gc[rr] = min(gc[rr], thresh + 1u);
-                    if (mn < 2u) {
-#pragma unroll
-                        for (int rr = 0; rr < R; ++rr)
-                            if (((mask >> rr) & 1) && cb[rr] >= thresh) slow(rr, tp[rr], gc[rr], pos, Uc);
-                    }
                     jf = __fadd2_rn(jf, f2(1.0f));
+                    return mn;
+                };
+                auto geomS = [&](int pos, auto MASK, SymGeo<R> &ge, auto Uc) {
+                    constexpr int mask = decltype(MASK)::value;
+#pragma unroll
+                    for (int rr = 0; rr < R; ++rr)
+                        if (((mask >> rr) & 1) && ge.cb[rr] >= thresh) slow(rr, ge.tp[rr], ge.c[rr], pos, Uc);
+                };
+                auto geom = [&](int pos, auto MASK, SymGeo<R> &ge, auto Uc) {
+                    if (geomA(MASK, ge) < 2u) geomS(pos, MASK, ge, Uc);
                 };
                 auto load = [&](int pos, auto MASK, const SymGeo<R> &ge, SymLd<R, B, NPL> &ld, auto Uc) {
                     const unsigned *gc = ge.c;
@@ -698,13 +709,29 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 constexpr bool PIPE = NC == 192 || (R == 3 && SC_R3_PIPE);                     // only the 6-warp instance needs it (elsewhere: spills, slower)
                 if (PLN) {
                     constexpr int kUn = SC_PLN_UNROLL;
+                    const std::integral_constant<int, 1> U1{};
 #pragma unroll 1
                     for (; pos + kUn - 1 <= plast; pos += kUn) {
-                        bodyu(pos, ALL, U0);
-                        bodyu(pos + 1, ALL, std::integral_constant<int, 1>{});
-                        if constexpr (kUn == 4) {
-                            bodyu(pos + 2, ALL, std::integral_constant<int, 2>{});
-                            bodyu(pos + 3, ALL, std::integral_constant<int, 3>{});
+                        if constexpr (SC_PLN_BATCH && kUn == 2) {
+                            // two positions as one straight-line block: both geometries, one branch for the rare exact
+                            // decisions, both sets of loads, both accumulations (the compiler cannot move position n + 1's
+                            // geometry across position n's branch by itself)
+                            const unsigned mA = geomA(ALL, geA), mB = geomA(ALL, geB);
+                            if (min(mA, mB) < 2u) {
+                                if (mA < 2u) geomS(pos, ALL, geA, U0);
+                                if (mB < 2u) geomS(pos + 1, ALL, geB, U1);
+                            }
+                            load(pos, ALL, geA, ldA, U0);
+                            load(pos + 1, ALL, geB, ldB, U1);
+                            fma(ALL, geA, ldA);
+                            fma(ALL, geB, ldB);
+                        } else {
+                            bodyu(pos, ALL, U0);
+                            bodyu(pos + 1, ALL, U1);
+                            if constexpr (kUn == 4) {
+                                bodyu(pos + 2, ALL, std::integral_constant<int, 2>{});
+                                bodyu(pos + 3, ALL, std::integral_constant<int, 3>{});
+                            }
                         }
                         adv(kUn);
                     }
