@@ -11,10 +11,13 @@
 //    NPL = (1 + SOUTH)(1 + MIRROR), each plane holding the 4 rotation images as one float4.
 //  * A persistent CTA works through tiles (runs of consecutive base pixels on one ring; several short runs
 //    of the rings near the pole are packed into one tile).  It is warp-specialised: producer warps stage, for every
-//    input ring within theta_max, the needed run of map values of every image into shared memory with 4-byte
-//    cp.async (the image runs are 4-byte-misaligned against each other, and the mirrored runs are reversed, which
-//    rules out TMA), reporting to full/empty mbarriers; the consumer warps (setmaxnreg gives them the producers'
-//    registers) run the pair loop.  No block-wide barrier after the prologue.
+//    input ring within theta_max, the needed run of map values of every image into shared memory, reporting to
+//    full/empty mbarriers; the consumer warps (setmaxnreg gives them the producers' registers) run the pair loop.
+//    No block-wide barrier after the prologue.  Two stage layouts: the 4 rotation images of a position interleaved
+//    as one float4, written with 4-byte cp.async (the image runs are 4-byte-misaligned against each other and the
+//    mirrored runs are reversed, which rules out TMA for this layout); or PLANAR (flag PLN, sc_sym_pl.cu: one map,
+//    small discs) -- one plane per image, filled by TMA bulk copies of 16-byte-aligned ring pieces, read with LDS.32
+//    by lanes kept exactly R positions apart (lane skew), two positions per straight-line block.
 //  * Pair geometry in fp32 without cancellation: t = A + B (1 - cos d) with A, B per ring pair from
 //    fp64, d = azimuth difference built from the INTEGER pixel offset (exact) times the ring's pixel
 //    spacing; 1 - cos d by a 4-term even polynomial (|d| <= ~0.9 rad on the rings this kernel takes;
