@@ -588,12 +588,11 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR")) cands.insert(cands.begin(), Cand{192, 4, true});
         // ... or 256 consumer threads x 3 base pixels: the same 768-pixel tiles with 8 consumer warps
         if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && !std::getenv("SC_SYM_NOR3")) cands.insert(cands.begin(), Cand{256, 3, true});
-        // ... with planar staging (one plane per image, TMA bulk copies; sc_sym_pl.cu) when the planes fit next to the table,
-        // for small discs (measured: config 3 sym kernel -8 %, config 4 -6 %; with the large-disc instance -- totals in tensor
-        // memory -- it came out SLOWER: Nside 2048 35' +4 %, 60' +12 %, Nside 1024 72' +8 %: the lanes' positions drift apart on
-        // distant input rings and their 4-byte loads then collide in the banks) and for maps with at least one full tile per
-        // SM (config 1: 0.031 against 0.022 ms, 64 tiny bulk copies per step)
-        if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && !std::getenv("SC_SYM_NOR3") && !std::getenv("SC_SYM_NOPLANAR") && mean_nb <= 700.0 &&
+        // ... with planar staging (one plane per image, TMA bulk copies, lane skew; sc_sym_pl.cu) when the planes fit next to
+        // the table, for discs of at most 2500 pixels (measured, sym kernel: config 3 -10 %, config 4 -10 %; with the
+        // tensor-memory totals of larger discs Nside 2048 35' -2.6 %, Nside 1024 72' -2 %, Nside 2048 60' +0.3 %) and for maps
+        // with at least one full tile per SM (config 1: 0.031 against 0.022 ms, 64 tiny bulk copies per step)
+        if (B == 1 && !std::getenv("SC_SYM_NOMIRROR") && !std::getenv("SC_SYM_NOR3") && !std::getenv("SC_SYM_NOPLANAR") && mean_nb <= 2500.0 &&
             tab_bytes + (size_t)kSymBufH * 16 * kPlanarPlane * 4 + 512 <= (size_t)smem_optin)
             cands.insert(cands.begin(), Cand{256, 3, true, false, true});
         // ... and as lane pairs (sc_sym_pair.cu): 32 accumulators per lane, 12 (small discs) or 8 consumer warps

@@ -289,7 +289,7 @@ def test_exact_integer_sums_fast_kernels(sc, nside, theta_am, ntab, B):
         assert bad.size == 0, (part, sel[bad[:10]], out[b][sel][bad[:10]], want[bad[:10]])
 
 
-@pytest.mark.parametrize("nside,theta_am,ntab", [(1024, 30, 8192), (1024, 40, 4096), (2048, 20, 16384)])
+@pytest.mark.parametrize("nside,theta_am,ntab", [(1024, 30, 8192), (1024, 72, 8192), (2048, 20, 16384)])
 def test_sym_staging_layouts_agree(sc, nside, theta_am, ntab, monkeypatch):
     """The 16-image sym kernel stages its input runs either as one plane per image by TMA bulk copies (the default,
     sc_sym_pl.cu; lanes skewed so that their 4-byte loads stay 3 positions apart) or as float4-interleaved rotation
