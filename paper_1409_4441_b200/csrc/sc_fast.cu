@@ -43,7 +43,7 @@ struct HostGeo {
 // all_rings: also the base rings that the belt kernel normally takes (north-cap-only convolution).
 // lanes: lanes of a warp that own a group of R base pixels each (32; 16 in the lane-pair instance).
 static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, int r_hi, int r_lo, bool mirror,
-                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32, int wcap = 0, int pad = 0) {
+                           std::vector<SymTile> &tiles, bool all_rings = false, int lanes = 32, int wcap = 0, int pad = 0, bool skew = false) {
     const int C = lanes * R;
     struct SubH { int r, k0, n, nw; int Lcap; double work; };
     auto make_sub = [&](int r, int k0, int n) {
@@ -52,7 +52,7 @@ static int build_sym_tiles(const HostGeo &g, int R, int W, int run, int Llimit, 
         const int klast = k0 + n - 1;
         for (const PairEnt &pe : g.per_ring[r]) {
             const int w0 = ((2 * k0 + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) - pe.hw;
-            const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0 + (pad > 0 ? 2 * pe.ex : 0);
+            const int L = ((2 * klast + 1 - sh) * pe.ipq + pe.shq * ip) / (2 * ip) + pe.hw + R - w0 + (skew ? 2 * pe.ex : 0);      // skew: runs staged ex positions further on both sides
             sb.Lcap = std::max(sb.Lcap, L);
             sb.work += (double)(2 * pe.hw + R);
         }
@@ -120,6 +120,7 @@ struct FastCfg {            // per batch size
     bool mirror = false;          // 16 images per pair geometry (reflection phi -> pi/2 - phi as well)
     bool pair = false;            // lane-pair instance: 16 lane pairs x R base pixels per warp
     bool planar = false;          // planar staging by TMA bulk copies (sc_sym_pl.cu)
+    bool skew = false;            // lane skew (planar and batch instances): longer staged runs
     std::map<std::pair<int, int>, std::pair<SymTile *, int>> band_tiles;   // (ring lo, hi) -> device tile list
     std::vector<int> ch_off, ch_lo, ch_hi;   // chunk i: tiles [ch_off[i], ch_off[i+1]), base rings ch_lo[i] .. ch_hi[i]
 };
@@ -206,7 +207,7 @@ cudaError_t fast_launch_band(FastPlan *fp, const Dev &P, const Maps &io, int B, 
         auto it = c.band_tiles.find({s_lo, s_hi});
         if (it == c.band_tiles.end()) {
             std::vector<SymTile> tiles;
-            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, c.mirror, tiles, false, c.pair ? 16 : 32, 0, c.planar ? kPlanarPad : 0);
+            const int Lneed = build_sym_tiles(*fp->geo, c.R, c.threads / 32, c.run, c.Ltot, s_hi, s_lo, c.mirror, tiles, false, c.pair ? 16 : 32, 0, c.planar ? kPlanarPad : 0, c.skew);
             if (Lneed > c.Ltot) return cudaErrorInvalidValue;
             SymTile *d = nullptr;
             if ((e = cudaMalloc((void **)&d, std::max<size_t>(tiles.size(), 1) * sizeof(SymTile))) != cudaSuccess) return e;
@@ -388,7 +389,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             PairEnt e;
             e.A = (float)(A64 * P.scale - 0.5);
             e.c1 = (float)(Bs / 2.0); e.c2 = (float)(-Bs / 24.0); e.c3 = (float)(Bs / 720.0); e.c4 = (float)(-Bs / 40320.0);
-            // lane skew of the planar sym instances (3 base pixels per lane): drift of 32 lanes against this ring, + 1;
+            // lane skew of the planar and batch sym instances (at most 3 base pixels per lane): drift of 32 lanes against this ring, + 1;
             // not worth it beyond 8 positions (rings next to the pole), not possible if the longer window would wrap
             e.ex = ipq == ip ? 0 : (int)std::ceil(31.0 * 3.0 * rho1) + 1;
             if (e.ex > 8 || ipq + 2 * hw + 2 * Rmax + 4 + 2 * e.ex >= 4 * ipq) e.ex = 0;
@@ -630,7 +631,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int Lmax = cd.planar ? kPlanarPlane : (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
             HostGeo &g = *fp->geo;
             g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;
-            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0, cd.planar ? kPlanarPad : 0); };
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0, cd.planar ? kPlanarPad : 0, cd.planar || B > 1); };
             // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
             // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
             std::vector<SymTile> tiles;
@@ -658,7 +659,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if (smem + stat > (size_t)smem_optin) continue;
             c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
             c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all; c.run = run;
-            c.mirror = cd.mirror; c.pair = cd.pair; c.planar = cd.planar;
+            c.mirror = cd.mirror; c.pair = cd.pair; c.planar = cd.planar; c.skew = cd.planar || B > 1;
             c.tmem = !cd.pair && (B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb > 700.0);      // large discs: two-level sums, totals in TMEM
             // a single accumulator set (plain fp32 running sums) only for one map and discs of at most 700 pixels
             c.tot = !(B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb <= 700.0);

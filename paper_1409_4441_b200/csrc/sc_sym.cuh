@@ -178,6 +178,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     constexpr int G = 2 * NPL;                           // float2 accumulators per base pixel and map
     constexpr int TMC = sym_tmem_cols(NC, R * G * 2);
     constexpr int NPD = SOUTH ? 2 : 1;                   // planes of direct images (the others: reflected)
+    constexpr bool SKEW = PLN || B > 1;                  // lane skew (see the consumers): runs staged PairEnt.ex positions further on both sides
     constexpr int NTASK = PLN ? 4 * NPL * kMaxSub : 0;   // planar staging: bulk-copy tasks (sub-tile, image) = producer threads that arrive
     static_assert(NTASK <= NPROD, "one producer thread per (sub-tile, image)");
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -244,7 +245,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 const unsigned M0s = 0xFFFFFFFFu / (unsigned)(2 * ips);
                 const int nq = 4 * ipq;
                 const int a0s = 2 * k0 + 1 - shs, als = 2 * (k0 + n - 1) + 1 - shs;
-                const int ex = PLN ? __ldg(&pe->ex) : 0;      // planar: extra positions on both sides (lane skew of the consumers)
+                const int ex = SKEW ? __ldg(&pe->ex) : 0;     // extra positions on both sides (lane skew of the consumers)
                 const int w0 = div_fast(a0s * ipq + shq * ips, 2 * ips, M0s, rem_unused) - hw - ex;
                 const int L = div_fast(als * ipq + shq * ips, 2 * ips, M0s, rem_unused) + hw + R + ex - w0;
                 int k = w0 + nq;                          // in [0, 2 nq): w0 >= -hw - 1 > -nq
@@ -441,7 +442,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
             if (step + 1 < me.ne) pe_next = F.pairs[me.e0 + step + 1];       // prefetch under the pair loop
             mbar_wait(&full_bar[buf], (it / kSymBuf) & 1u);
             if (active && step < me.ne && !(F.dbg & 1)) {
-                const int ex = PLN ? pe.ex : 0;
+                const int ex = SKEW ? pe.ex : 0;
                 const int w0 = div_fast(ap0 * pe.ipq + pe.shq * ip, ip2, M0, rem_unused) - pe.hw - ex;
                 int rem;
                 const int kc = div_fast(ap * pe.ipq + pe.shq * ip, ip2, M0, rem);
@@ -539,20 +540,22 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                 float2 dc2[RP];
 #pragma unroll
                 for (int h = 0; h < RP; ++h) dc2[h] = f2(dcr[2 * h], dcr[2 * h + 1 < R ? 2 * h + 1 : 2 * h]);
-                // Planar staging, lane skew: on an input ring with another pixel count the lanes' positions, R apart on the base
-                // ring, drift apart by up to ex and their 4-byte loads would collide in the banks.  A lane whose position is
+                // Lane skew (planar and batch instances): on an input ring with another pixel count the lanes' positions, R apart
+                // on the base ring, drift apart by up to ex and their loads would collide in the banks.  A lane whose position is
                 // `skew` ahead of the grid (first valid lane's position + R per lane, shifted to the smallest) starts its walk
                 // `skew` positions early and all lanes walk 2 hw + R + wd positions (wd = the largest skew of the warp): at
                 // every step the valid lanes are exactly R positions apart.  The extra positions lie outside the disc (weight
                 // 0) and inside the staged run (extended by ex on both sides).
                 int skew = 0, wd = 0;
-                if (PLN && ex > 0) {
+                if (SKEW && ex > 0) {
                     const bool valid = kmine <= klast;
                     const int q = i0 - R * lane;
                     const int mn = __reduce_min_sync(0xFFFFFFFFu, valid ? q : 0x7FFFFFFF);
                     const int mx = __reduce_max_sync(0xFFFFFFFFu, valid ? q : (int)0x80000000);
-                    skew = valid ? q - mn : 0;
-                    wd = mx - mn;
+                    if (mx - mn <= ex) {                          // (always, by the choice of ex; else: no skew, the run is not that long)
+                        skew = valid ? q - mn : 0;
+                        wd = mx - mn;
+                    }
                 }
                 float2 jf = f2((float)(-pe.hw - skew));
                 const int pos0 = i0 - pe.hw - skew, pend = i0 + pe.hw + R - 1 + wd - skew;
