@@ -255,7 +255,7 @@ cudaError_t fast_launch_cap(FastPlan *fp, const Dev &P, const Maps &io, int ring
             const int W = cd.threads / 32, C = 32 * cd.R;
             for (int shrink = 0; shrink <= W * C / 4 && !c.ok; shrink += 16) {
                 tiles.clear();
-                const int Lneed = build_sym_tiles(*fp->geo, cd.R, W, W * C - shrink, Lmax, s_hi, s_lo, true, tiles, true);
+                const int Lneed = build_sym_tiles(*fp->geo, cd.R, W, W * C - shrink, Lmax, s_hi, s_lo, true, tiles, true, 32, 0, 0, true);
                 const size_t smem = fp->tab_bytes + (size_t)kSymBufH * 2 * Lneed * 16;
                 if (smem + 512 > (size_t)fp->smem_optin) continue;
                 c.threads = cd.threads; c.R = cd.R; c.run = W * C - shrink; c.mirror = true; c.Ltot = Lneed; c.smem = smem;
@@ -631,7 +631,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             const int Lmax = cd.planar ? kPlanarPlane : (int)(((size_t)smem_optin - stat - tab_bytes) / ((size_t)kSymBufH * B * npl * 16)) & ~7;
             HostGeo &g = *fp->geo;
             g.N = N; g.polar = polar; g.per_ring = per_ring; g.slot_of = slot_of; g.pair_off = pair_off; g.is_belt = is_belt;
-            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0, cd.planar ? kPlanarPad : 0, cd.planar || B > 1); };
+            auto build = [&](int r_hi, int r_lo, std::vector<SymTile> &tl) { return build_sym_tiles(g, R, W, run, Lmax, r_hi, r_lo, cd.mirror, tl, false, cd.pair ? 16 : 32, shrink0 > 0 ? (run + C - 1) / C : 0, cd.planar ? kPlanarPad : 0, true); };
             // (1) the whole range in one work-sorted list: sc_convolve; (2) the same rings in kSymChunks
             // latitude chunks from the belt towards the pole, each sorted: the pipelined host entry
             std::vector<SymTile> tiles;
@@ -659,7 +659,7 @@ FastPlan *fast_plan_create(const Dev &P, const std::vector<double> &z, const std
             if (smem + stat > (size_t)smem_optin) continue;
             c.ntiles_all = ch_off[0]; c.ch_off = ch_off; c.ch_lo = ch_lo; c.ch_hi = ch_hi;
             c.threads = cd.threads; c.R = R; c.Ltot = Ltot; c.smem = smem; c.ntiles = c.ntiles_all; c.run = run;
-            c.mirror = cd.mirror; c.pair = cd.pair; c.planar = cd.planar; c.skew = cd.planar || B > 1;
+            c.mirror = cd.mirror; c.pair = cd.pair; c.planar = cd.planar; c.skew = true;
             c.tmem = !cd.pair && (B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb > 700.0);      // large discs: two-level sums, totals in TMEM
             // a single accumulator set (plain fp32 running sums) only for one map and discs of at most 700 pixels
             c.tot = !(B == 1 && (cd.threads == 384 || cd.mirror) && mean_nb <= 700.0);

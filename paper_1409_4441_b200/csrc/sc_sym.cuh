@@ -108,6 +108,10 @@ constexpr int kSymBuf = 2;        // stage buffers
 #ifndef SC_R3_PIPE
 #define SC_R3_PIPE 0
 #endif
+// lane skew in every instance (0: only the planar and the batch instances)
+#ifndef SC_SKEW_ALL
+#define SC_SKEW_ALL 1
+#endif
 #ifndef SC_SYM_BATCH
 #define SC_SYM_BATCH 1
 #endif
@@ -178,7 +182,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
     constexpr int G = 2 * NPL;                           // float2 accumulators per base pixel and map
     constexpr int TMC = sym_tmem_cols(NC, R * G * 2);
     constexpr int NPD = SOUTH ? 2 : 1;                   // planes of direct images (the others: reflected)
-    constexpr bool SKEW = PLN || B > 1;                  // lane skew (see the consumers): runs staged PairEnt.ex positions further on both sides
+    constexpr bool SKEW = SC_SKEW_ALL || PLN || B > 1;                  // lane skew (see the consumers): runs staged PairEnt.ex positions further on both sides
     constexpr int NTASK = PLN ? 4 * NPL * kMaxSub : 0;   // planar staging: bulk-copy tasks (sub-tile, image) = producer threads that arrive
     static_assert(NTASK <= NPROD, "one producer thread per (sub-tile, image)");
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -557,6 +561,7 @@ sym_kernel(const Dev P, const FastDev F, const Maps io) {
                         wd = mx - mn;
                     }
                 }
+                if (HP) jd = -(double)(pe.hw + skew);
                 float2 jf = f2((float)(-pe.hw - skew));
                 const int pos0 = i0 - pe.hw - skew, pend = i0 + pe.hw + R - 1 + wd - skew;
                 // One window position for the pixels rr in MASK (compile time).  The window of the thread is the
