@@ -271,8 +271,12 @@ def _roofline(cfg, B, total_pairs, kern_ms, kern_pairs, step_ms, step_min_ms, no
     step_ops = sum(per_kernel[k]["executed_fp32_ops"] for k in counted) if all_exec else None
     lim = None
     if d.get("smem_pipe_pct_ncu") is not None and d.get("fma_pipe_active_pct_ncu") is not None:
-        lim = ("shared-memory pipe" if d["smem_pipe_pct_ncu"] > d["fma_pipe_active_pct_ncu"] else "FMA pipe") + \
-              f" (ncu: shared-memory wavefronts {d['smem_pipe_pct_ncu']:.0f} %, FMA pipe {d['fma_pipe_active_pct_ncu']:.0f} % of peak)"
+        busiest = max(d["smem_pipe_pct_ncu"], d["fma_pipe_active_pct_ncu"])
+        # below ~70 % of every pipe the kernel waits on dependent-issue latency (few warps per scheduler), not on a pipe
+        lim = ("latency (no pipe saturated)" if busiest < 70.0 else
+               "shared-memory pipe" if d["smem_pipe_pct_ncu"] > d["fma_pipe_active_pct_ncu"] else "FMA pipe") + \
+              f" (ncu: shared-memory wavefronts {d['smem_pipe_pct_ncu']:.0f} %, FMA pipe {d['fma_pipe_active_pct_ncu']:.0f} %" + \
+              (f", issue slots {d['issue_active_pct_ncu']:.0f} %" if d.get("issue_active_pct_ncu") is not None else "") + " of peak)"
     return {
         "bound": "alu", "kernel": dom, "achieved": achieved / 1e9, "peak": measured / 1e9, "unit": "GFMA/s",
         "frac": achieved / measured,
